@@ -1,0 +1,348 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only).
+
+Each test is chosen so that a plausible mistake in oracle/sk_oracle.cpp (a dropped term, a wrong
+sign, index or offset, un-normalised pooling, Eq. 13 instead of Eq. 14) fails at least one.
+PAPER.md line numbers refer to /root/reference/PAPER.md (arXiv 1808.10365).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def enc(re, im):
+    """Encode integer components in [-8, 7] (test-side helper; the inverse of the method's a1)."""
+    return (((np.asarray(re) + 8) << 4) | (np.asarray(im) + 8)).astype(np.uint8)
+
+
+# ---------------------------------------------------------------------------------------- P7
+def test_hand_example_golden(oracle):
+    """Hand-worked sums, tests/golden/hand_example.txt (PAPER.md:77 Eq. 7, :108-113 Eq. 14)."""
+    kv = {}
+    for line in open(os.path.join(GOLDEN, "hand_example.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, *v = line.split()
+        kv[k] = v
+    M, E = int(kv["M"][0]), int(kv["E"][0])
+    data = np.array([int(x, 16) for x in kv["data"]], np.uint8).reshape(M, 1, E)
+    S1, S2 = oracle.power_sums(data, M)
+    assert S1.ravel().tolist() == [int(x) for x in kv["S1"]]
+    assert S2.ravel().tolist() == [int(x) for x in kv["S2"]]
+    sk2, sk64 = oracle.combine(S1, S2, M, want64=True)
+    assert sk64[0, 0] == float(kv["SK_N2"][0])          # 0.3125 is exact in binary
+    assert sk2[0, 0] == np.float32(kv["SK_N2"][0])
+    assert oracle.combine(S1, S2, M, first_n=1)[0, 0] == np.float32(kv["SK_input0"][0])
+    assert oracle.combine(S1, S2, M, subset=[0, 1])[0, 0] == np.float32(kv["SK_input1"][0])
+    assert oracle.single(8, 22, 4) == 0.625             # Eq. 2 on the same sums
+
+
+def test_decode_offsets(oracle):
+    """a1: value = nibble - 8, nibble 0 decodes to -8 (reading A3), 0x88 is zero."""
+    M = 2
+    for byte, p in [(0x88, 0), (0x00, 128), (0xFF, 98), (0x80, 64), (0x08, 64), (0x8F, 49),
+                    (0xF8, 49), (0x97, 2), (0x11, 98), (0x10, 49 + 64)]:
+        data = np.full((M, 1, 1), byte, np.uint8)
+        S1, S2 = oracle.power_sums(data, M)
+        assert (S1[0, 0, 0], S2[0, 0, 0]) == (M * p, M * p * p), hex(byte)
+
+
+# ---------------------------------------------------------------------------------------- P1
+@pytest.mark.parametrize("M,E", [(4, 1), (64, 16), (256, 256), (1024, 48)])
+def test_constant_modulus_gives_exactly_zero(oracle, M, E):
+    """A constant-modulus signal has M*S2/S1^2 = 1 exactly, so Eq. 2 / Eq. 14 give 0 exactly."""
+    rng = np.random.default_rng(1)
+    pts = np.array([(5, 0), (-5, 0), (0, 5), (0, -5), (3, 4), (-3, 4), (3, -4), (-3, -4),
+                    (4, 3), (-4, 3), (4, -3), (-4, -3)])
+    k = rng.integers(0, len(pts), size=(3 * M, 2, E))
+    data = enc(pts[k, 0], pts[k, 1])
+    r = oracle.frame(data, M)
+    assert (r["S1"] == 25 * M).all() and (r["S2"] == 625 * M).all()
+    assert (r["SK"] == 0.0).all()
+    # |0 - 1| is outside 3 sigma exactly when 3*sqrt(4/(MN)) < 1
+    assert (r["mask"] == (1 if 3 * math.sqrt(4 / (M * E)) < 1 else 0)).all()
+
+
+# ---------------------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("scale,lim", [(2, 3), (3, 2)])
+def test_scale_invariance_is_exact(oracle, scale, lim):
+    """'overall-scaling-invariant': S2/S1^2 is a ratio of degree-4 forms, and on the
+    integer grid scaling by k multiplies both exactly, so SK64 is bit-identical."""
+    rng = np.random.default_rng(2)
+    M, F, E = 32, 3, 24
+    re = rng.integers(-lim, lim + 1, size=(4 * M, F, E))
+    im = rng.integers(-lim, lim + 1, size=(4 * M, F, E))
+    re[:, :, 0] = np.where(re[:, :, 0] == 0, 1, re[:, :, 0])     # keep every input's power > 0
+    a = oracle.frame(enc(re, im), M)
+    b = oracle.frame(enc(scale * re, scale * im), M)
+    assert (b["S1"] == scale ** 2 * a["S1"]).all() and (b["S2"] == scale ** 4 * a["S2"]).all()
+    ska = oracle.combine(a["S1"], a["S2"], M, want64=True)[1]
+    skb = oracle.combine(b["S1"], b["S2"], M, want64=True)[1]
+    # the quotient M^2 S2 / S1^2 is the same real number; both operand pairs are exact in double
+    np.testing.assert_array_equal(ska, skb)
+
+
+# ---------------------------------------------------------------------------- P3, P4, P5, Eq. 12
+def test_paper_identities(oracle):
+    """S1bar = nN (Eq. 10), Eq. 12, Eq. 14's second and third lines agree, Eq. 13/14 ratio."""
+    rng = np.random.default_rng(3)
+    M, F, E = 64, 2, 40
+    data = rng.integers(0, 256, size=(5 * M, F, E), dtype=np.uint8)
+    S1, S2 = oracle.power_sums(data, M)
+    for kw in (dict(), dict(first_n=7), dict(subset=(np.arange(E) % 3 == 1))):
+        N = E if not kw else (7 if "first_n" in kw else int(np.count_nonzero(kw["subset"])))
+        sk32, sk = oracle.combine(S1, S2, M, want64=True, **kw)
+        avg = oracle.average_of_singles(S1, S2, M, **kw)
+        sk13, s1bar, s2bar = oracle.eq13_and_s1bar(S1, S2, M, **kw)
+        np.testing.assert_allclose(s1bar, M * N, rtol=1e-13)                       # Eq. 10
+        np.testing.assert_allclose(sk, avg, rtol=1e-12, atol=1e-14)                # Eq. 14 l.2 = l.3
+        np.testing.assert_allclose(s2bar, M * (M - 1) / (M + 1) * N * avg + M * N,
+                                   rtol=1e-12)                                     # Eq. 12
+        ratio = (M * N + 1) * (M - 1) / ((M * N - 1) * (M + 1))
+        np.testing.assert_allclose(sk13, ratio * sk, rtol=1e-12)                   # Eq. 13 vs 14
+        np.testing.assert_array_equal(sk32, sk.astype(np.float32))
+
+
+def test_n1_reduces_to_single_receiver(oracle):
+    """N = 1: Eq. 14 is Eq. 2."""
+    rng = np.random.default_rng(4)
+    M = 16
+    data = rng.integers(0, 256, size=(3 * M, 1, 5), dtype=np.uint8)
+    S1, S2 = oracle.power_sums(data, M)
+    for e in range(5):
+        sub = np.arange(5) == e
+        sk = oracle.combine(S1, S2, M, subset=sub, want64=True)[1]
+        for b in range(3):
+            assert sk[b, 0] == pytest.approx(oracle.single(S1[b, 0, e], S2[b, 0, e], M), rel=1e-14)
+
+
+def test_two_level_closed_form(oracle):
+    """A receiver alternating between powers a and b has M S2/S1^2 = 2(a^2+b^2)/(a+b)^2:
+    with a=1 (0x98), b=4 (0xA8): 2*17/25 = 1.36, SK = (M+1)/(M-1)*0.36."""
+    M = 10
+    data = np.array([0x98, 0xA8] * (M // 2), np.uint8).reshape(M, 1, 1)
+    sk = oracle.frame(data, M)["SK"][0, 0]
+    assert sk == np.float32(11 / 9 * 0.36)
+
+
+# --------------------------------------------------------------------------------------- P12
+def brute(data, M, sel):
+    """Differently structured: per-input Eq. 8 with Python ints/Fractions, then the average."""
+    from fractions import Fraction
+    T, F, E = data.shape
+    out = np.zeros((T // M, F))
+    for b in range(T // M):
+        for f in range(F):
+            tot = Fraction(0)
+            for e in sel:
+                ps = []
+                for t in range(b * M, (b + 1) * M):
+                    byte = int(data[t, f, e])
+                    hi, lo = divmod(byte, 16)
+                    ps.append((hi - 8) ** 2 + (lo - 8) ** 2)
+                s1, s2 = sum(ps), sum(p * p for p in ps)
+                if s1:
+                    tot += Fraction(M + 1, M - 1) * (Fraction(M * s2, s1 * s1) - 1)
+            out[b, f] = float(tot / len(sel))
+    return out
+
+
+@pytest.mark.parametrize("M,E", [(2, 1), (3, 4), (8, 8), (5, 7)])
+def test_brute_force_tiny(oracle, M, E):
+    rng = np.random.default_rng(100 + M)
+    data = rng.integers(0, 256, size=(4 * M, 2, E), dtype=np.uint8)
+    data[:, 0, 0] = 0x88                  # a dead input (reading A4)
+    data[:M, 1, :] = rng.choice([0x00, 0x08, 0x80, 0x88, 0xFF], size=(M, E))  # nibble 0 = -8
+    for sel in (list(range(E)), list(range(0, E, 2))):
+        sub = np.isin(np.arange(E), sel)
+        sk = oracle.combine(*oracle.power_sums(data, M), M, subset=sub, want64=True)[1]
+        np.testing.assert_allclose(sk, brute(data, M, sel), rtol=1e-13, atol=1e-14)
+
+
+def test_all_zero_cell_is_zero_and_flagged(oracle):
+    """Reading A4: an all-0x88 cell gives SK = 0 exactly (no NaN) and is flagged."""
+    data = np.full((128, 2, 16), 0x88, np.uint8)
+    r = oracle.frame(data, 64)
+    assert (r["SK"] == 0).all() and (r["mask"] == 1).all() and not np.isnan(r["SK"]).any()
+
+
+# --------------------------------------------------------------------------------------- P11
+def test_permutations(oracle):
+    rng = np.random.default_rng(5)
+    M, F, E = 32, 2, 64
+    data = rng.integers(0, 256, size=(2 * M, F, E), dtype=np.uint8)
+    S1, S2 = oracle.power_sums(data, M)
+    shuf = data.copy()
+    for b in range(2):
+        shuf[b * M:(b + 1) * M] = data[b * M + rng.permutation(M)]
+    S1s, S2s = oracle.power_sums(shuf, M)
+    assert (S1 == S1s).all() and (S2 == S2s).all()          # time order inside a block is irrelevant
+    perm = rng.permutation(E)
+    a = oracle.combine(S1, S2, M, want64=True)[1]
+    b = oracle.combine(S1[:, :, perm], S2[:, :, perm], M, want64=True)[1]
+    np.testing.assert_allclose(a, b, rtol=1e-13)             # input order: only rounding changes
+    swapped = data.copy()
+    swapped[:M], swapped[M:] = data[M:], data[:M]            # blocks are independent (A10)
+    c = oracle.frame(swapped, M)["SK"]
+    np.testing.assert_array_equal(c[::-1], oracle.frame(data, M)["SK"])
+
+
+# ---------------------------------------------------------------------------------------- P8
+def _gauss(rng, T, F, E, sig):
+    return rng.standard_normal((T, F, E)) * sig, rng.standard_normal((T, F, E)) * sig
+
+
+@pytest.mark.parametrize("M,N,cells", [(64, 8, 20000), (256, 4, 6000)])
+def test_null_moments_float_input(oracle, M, N, cells):
+    """Circular Gaussian input: mean(SK~) = 1 (Eq. 15), var(SK~) = 4/(nN) + O(1/(n^2 N)) (Eq. 16).
+    Per-input sigma varies by 2.3x, so pooling un-normalised sums would fail this test."""
+    rng = np.random.default_rng(8)
+    sig = rng.uniform(1.5, 3.5, size=N)
+    re, im = _gauss(rng, M * cells, 1, N, sig)
+    sk = oracle.frame_float(re, im, M)[0].ravel()
+    first = 4.0 / (M * N)
+    se_mean = math.sqrt(first / cells)
+    assert abs(sk.mean() - 1.0) < 4 * se_mean
+    # exact Gaussian-input variance is 4 M^2 / ((M-1)(M+2)(M+3) N): first order minus O(1/M)
+    ratio = sk.var(ddof=1) / first
+    expected = M ** 3 / ((M - 1) * (M + 2) * (M + 3))
+    assert abs(ratio - expected) < 4 * math.sqrt(2.0 / cells) + 0.01
+    assert abs(ratio - 1.0) < 6.0 / M + 4 * math.sqrt(2.0 / cells)      # "to first order"
+    # the wrong estimator (Eq. 13, un-rescaled) is biased low by (nN+1)(n-1)/((nN-1)(n+1))
+    assert abs(sk.mean() * (M * N + 1) * (M - 1) / ((M * N - 1) * (M + 1)) - 1.0) > 4 * se_mean
+
+
+def test_unnormalised_pooling_would_fail(oracle):
+    """Control for P8: pooling raw S1, S2 across receivers of unequal power is NOT mean-1."""
+    rng = np.random.default_rng(9)
+    M, N, cells = 64, 8, 4000
+    sig = np.linspace(1.0, 4.0, N)
+    re, im = _gauss(rng, M * cells, 1, N, sig)
+    sk, S1, S2 = oracle.frame_float(re, im, M)
+    pooled = (M * N + 1) / (M * N - 1) * (M * N * S2.sum(-1) / S1.sum(-1) ** 2 - 1)
+    assert abs(pooled.mean() - 1.0) > 0.3 and abs(sk.mean() - 1.0) < 0.01
+
+
+# ---------------------------------------------------------------------------------------- P9
+def test_skew_and_kurtosis_single_receiver(oracle):
+    """N = 1: skew ~ 10/sqrt(M), excess kurtosis ~ 246/M to first order."""
+    rng = np.random.default_rng(10)
+    M, cells = 128, 100000
+    re, im = _gauss(rng, M * cells // 50, 1, 50, 2.0)      # 50 independent receivers, used singly
+    _, S1, S2 = oracle.frame_float(re, im, M)
+    sk = (M + 1) / (M - 1) * (M * S2 / S1 ** 2 - 1)
+    sk = sk.ravel()
+    assert sk.size == cells
+    d = sk - sk.mean()
+    skew = (d ** 3).mean() / (d ** 2).mean() ** 1.5
+    kurt = (d ** 4).mean() / (d ** 2).mean() ** 2 - 3.0
+    assert abs(sk.mean() - 1) < 4 * math.sqrt(4 / M / cells)
+    assert abs(sk.var() / (4 / M) - 1) < 0.08
+    assert abs(skew / (10 / math.sqrt(M)) - 1) < 0.30
+    assert abs(kurt / (246 / M) - 1) < 0.35
+
+
+# --------------------------------------------------------------------------------------- P10
+def test_digitised_offset_is_constant_in_N(oracle):
+    """App. B: 4+4-bit data, RMS 1.52 LSB, clipped to +-7: the mean of SK~
+    converges to a constant slightly off 1 for all N, the variance to the float-input value."""
+    rng = np.random.default_rng(11)
+    M, E, cells = 256, 64, 1500
+    re = np.clip(np.rint(rng.standard_normal((M * cells, 1, E)) * 1.52), -7, 7).astype(int)
+    im = np.clip(np.rint(rng.standard_normal((M * cells, 1, E)) * 1.52), -7, 7).astype(int)
+    S1, S2 = oracle.power_sums(enc(re, im), M)
+    means = {}
+    for N in (4, 16, 64):
+        sk = oracle.combine(S1, S2, M, first_n=N, want64=True)[1].ravel()
+        means[N] = sk.mean()
+        se = math.sqrt(4 / (M * N) / cells)
+        assert abs(sk.mean() - 1) < 0.01                      # "slightly offset from unity"
+        assert abs(sk.var() / (4 / (M * N)) - 1) < 0.15       # variance as in the float case
+        assert abs(means[N] - means[4]) < 5 * math.sqrt(4 / (M * 4) / cells) + se
+    assert means[64] < 1.0                                    # the offset is real (about -1e-3)
+    # large-M limit from the quantised pmf alone: E[p^2]/E[p]^2 - 1 (finite-M bias is O(1/M))
+    assert abs(means[64] - _quantised_limit(1.52)) < 4 * math.sqrt(4 / (M * 64) / cells) + 2.0 / M
+
+
+def _quantised_limit(sigma):
+    """E[p^2]/E[p]^2 - 1 for p = re^2 + im^2 with re, im iid rounded-and-clipped N(0, sigma^2):
+    computed from the normal cdf, with no reference to the estimator's code."""
+    k = np.arange(-7, 8)
+    cdf = lambda x: 0.5 * (1 + np.vectorize(math.erf)(x / (sigma * math.sqrt(2))))
+    pmf = cdf(k + 0.5) - cdf(k - 0.5)
+    pmf[0] += cdf(-7.5)
+    pmf[-1] += 1 - cdf(7.5)
+    m2, m4 = (pmf * k ** 2).sum(), (pmf * k ** 4).sum()
+    return (2 * m4 + 2 * m2 * m2) / (2 * m2) ** 2 - 1
+
+
+def test_digitised_mean_matches_pmf_prediction(oracle):
+    """sigma = 2.5 LSB clipped at +-7 (configs 0 and 3): the null mean of SK~ on 4-bit data sits
+    well below 1 (about 0.94); its large-M limit follows from the quantised pmf."""
+    rng = np.random.default_rng(13)
+    M, E, cells = 256, 128, 400
+    re = np.clip(np.rint(rng.standard_normal((M * cells, 1, E)) * 2.5), -7, 7).astype(int)
+    im = np.clip(np.rint(rng.standard_normal((M * cells, 1, E)) * 2.5), -7, 7).astype(int)
+    sk = oracle.frame(enc(re, im), M)["SK"].ravel().astype(np.float64)
+    lim = _quantised_limit(2.5)
+    assert 0.92 < lim < 0.96
+    assert abs(sk.mean() - lim) < 4 * math.sqrt(4 / (M * E) / cells) + 2.0 / M
+
+
+# -------------------------------------------------------------------------------------- flag
+def test_flag_interval(oracle):
+    """flagged iff outside mean +- a*sqrt(var); var = 4/(nN) (Eq. 16); strict; NaN."""
+    M, N, a = 256, 2048, 5.0
+    s = math.sqrt(4.0 / (M * N))
+    mean = 0.9985
+    SK = np.array([[mean, mean + 4.99 * s, mean + 5.01 * s, mean - 4.99 * s, mean - 5.01 * s,
+                    np.nan, np.inf, 0.0, 2.0]], np.float32)
+    m = oracle.flag(SK, M, N, a, sk_mean=mean)
+    assert m.tolist() == [[0, 0, 1, 0, 1, 1, 1, 1, 1]]
+    thr = np.float32(a * s)
+    edge = np.array([[np.float32(1.0) + thr, np.float32(1.0) - thr]], np.float32)
+    dev = np.abs(edge - np.float32(1.0))
+    assert (oracle.flag(edge, M, N, a, sk_mean=1.0) == (dev > thr)).all()     # strict, in float32
+    # the width scales as 1/sqrt(N): 4x the receivers, half the interval
+    assert oracle.flag(np.array([[1 + 2.6 * s]], np.float32), M, N, a)[0, 0] == 0
+    assert oracle.flag(np.array([[1 + 2.6 * s]], np.float32), M, 4 * N, a)[0, 0] == 1
+
+
+def test_frame_excision(oracle):
+    """Reading A11: flagged cells (all E inputs, all M rows) become 0x88, others are untouched;
+    mask and SK come from the data before excision; a second pass is idempotent (A4)."""
+    rng = np.random.default_rng(12)
+    M, F, E = 64, 3, 32
+    re = np.clip(np.rint(rng.standard_normal((4 * M, F, E)) * 1.5), -7, 7).astype(int)
+    im = np.clip(np.rint(rng.standard_normal((4 * M, F, E)) * 1.5), -7, 7).astype(int)
+    re[M:2 * M, 1, :] = 5
+    im[M:2 * M, 1, :] = 0                                     # cell (1,1): constant modulus
+    data = enc(re, im)
+    null_mean = float(oracle.frame(data, M)["SK"][[0, 2, 3]].mean())
+    r = oracle.frame(data, M, n_sigma=6.0, sk_mean=null_mean, zero_flagged=True)
+    assert r["mask"][1, 1] == 1 and r["mask"].sum() == 1
+    expect = data.copy()
+    expect[M:2 * M, 1, :] = 0x88
+    np.testing.assert_array_equal(r["data"], expect)
+    plain = oracle.frame(data, M, n_sigma=6.0, sk_mean=null_mean)
+    np.testing.assert_array_equal(plain["SK"], r["SK"])
+    np.testing.assert_array_equal(plain["data"], data)
+    again = oracle.frame(r["data"], M, n_sigma=6.0, sk_mean=null_mean, zero_flagged=True)
+    assert again["SK"][1, 1] == 0 and again["mask"][1, 1] == 1
+    np.testing.assert_array_equal(again["data"], r["data"])
+
+
+def test_bad_arguments(oracle):
+    d = np.zeros((8, 1, 4), np.uint8)
+    with pytest.raises(ValueError):
+        oracle.power_sums(d, 3)            # T % M != 0
+    with pytest.raises(ValueError):
+        oracle.power_sums(d, 1)            # M < 2
+    S1, S2 = oracle.power_sums(d, 4)
+    with pytest.raises(ValueError):
+        oracle.combine(S1, S2, 4, first_n=5)   # N > E
+    with pytest.raises(ValueError):
+        oracle.combine(S1, S2, 4, subset=[0, 0, 0, 0])   # N == 0
