@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fused SK hot path (arXiv 1808.10365) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg1|cfg4|...]
+
+A step is one pass of the whole hot path (unpack -> S1/S2 -> Eq. 14 -> flag) over one synthetic
+frame of the workload.  Metric: SK input samples/s (1 sample = 1 byte of 4+4-bit data), whole job.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sk_input_samples_per_s"
+UNIT = "samples/s"
+FALLBACK_HBM_GBS = 6650.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--no-graph", action="store_true", help="launch step by step instead of one CUDA graph")
+    ap.add_argument("--zero", action="store_true", help="excise flagged cells in place (a8)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(name):
+    import sk_synth
+    idx = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4}[name]
+    return sk_synth.config(idx)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def stored_traffic(cfg_name):
+    """dram bytes per launch from the committed ncu --set full capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+            return json.load(f).get(cfg_name, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.stop_flag, self.ok = [], set(), False, False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+        self.window = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+        } if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else {
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+        }
+        while not self.stop_flag:
+            try:
+                t = time.perf_counter()
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.samples.append((t, mhz, r))
+                for bit, nm in names.items():
+                    if r & bit and self.window and self.window[0] <= t <= (self.window[1] or 1e30):
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.0005)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        lo, hi = self.window if self.window else (0, 1e30)
+        inside = sorted(m for (t, m, _) in self.samples if lo <= t <= (hi or 1e30))
+        allv = sorted(m for (_, m, _) in self.samples)
+        use = inside if inside else allv
+        return {"sm_mhz": use[len(use) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(inside)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores, on the same workload/metric.
+    Each step is one full frame of the workload when that fits a few seconds, else a slab of blocks."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import sk_synth
+    from oracle import sk_oracle
+    cfg = workload(args.workload)
+    # bounded sample: at ~0.2 Gsamples/s keep one step near half a second
+    max_bytes = 100 * 1024 * 1024
+    blocks = max(1, min(cfg.B, max_bytes // (cfg.M * cfg.F * cfg.E)))
+    sub = cfg.with_(T=blocks * cfg.M)
+    host = sk_synth.make_frame(sub).numpy()
+    steps = max(1, min(args.steps, 20))
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
+        sk_oracle.frame(host, cfg.M, n_sigma=cfg.n_sigma)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        sk_oracle.frame(host, cfg.M, n_sigma=cfg.n_sigma)
+    dt = time.perf_counter() - t0
+    v = host.size * steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M,
+                   "sample": f"{blocks} of {cfg.B} blocks per step ({host.size} samples)"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"{steps} steps x {host.size} samples of {cfg.name}"},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the SK path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    sk.lib()
+
+    cfg = workload(args.workload)
+    K, W = args.steps, max(args.warmup, 3)
+    frame_bytes = cfg.nbytes
+    # distinct frames so that no step re-reads L2-resident data: > 4x the 126 MB L2, or 10 frames
+    l2 = 126 * 1024 * 1024
+    nbuf = 10 if frame_bytes > l2 else max(4, -(-5 * l2 // frame_bytes))
+    free = torch.cuda.mem_get_info()[0]
+    nbuf = max(2, min(nbuf, int(free * 0.8) // frame_bytes))
+    # every rank draws its own frames (weak scaling: independent frames per GPU, no collective)
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=rank * 1000 + i) for i in range(nbuf)]
+    null = sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * cfg.M), cw_block_inputs=None, cw_freqs=(),
+                                         burst_fraction=0.0, sine_freqs=()), device=dev, frame=777)
+    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())     # null mean on 4-bit data
+    n_sigma = 5.0
+    outs = [sk.sk_frame(b, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean) for b in bufs[:1]]
+    out = outs[0]
+    ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, 0)
+    stream = torch.cuda.Stream(device=dev)
+    pristine = [b.clone() for b in bufs] if args.zero and nbuf * frame_bytes * 2 < free * 0.8 else None
+
+    def step(i):
+        sk.sk_frame(bufs[i % nbuf], cfg.M, n_sigma=n_sigma, sk_mean=sk_mean, zero_flagged=args.zero,
+                    out=out, workspace=ws, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    with torch.cuda.stream(stream):
+        for i in range(W):
+            step(i)
+    torch.cuda.synchronize()
+    flagged = float(out.mask.float().mean().item())
+
+    graph = None
+    n0 = sk.sk_launch_count()
+    if not args.no_graph:
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for i in range(K):
+                step(i)
+        launches = sk.sk_launch_count() - n0
+        with torch.cuda.stream(stream):
+            graph.replay()                      # one untimed replay (graph upload)
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_lo = time.perf_counter()
+    sampler.window = (t_lo, None)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        if graph is not None:
+            graph.replay()
+        else:
+            n0 = sk.sk_launch_count()
+            for i in range(K):
+                step(i)
+            launches = sk.sk_launch_count() - n0
+        e1.record(stream)
+    barrier()
+    sampler.window = (t_lo, time.perf_counter())
+    ms = e0.elapsed_time(e1)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+
+    # ---- end to end through the C ABI with host buffers (copies inside the timed region)
+    Ke = args.e2e_steps or min(K, 20)
+    h_frames = [bufs[i % nbuf].cpu().pin_memory() for i in range(min(2, nbuf))]
+    h_SK = torch.empty(cfg.B, cfg.F, dtype=torch.float32).pin_memory()
+    h_mask = torch.empty(cfg.B, cfg.F, dtype=torch.uint8).pin_memory()
+    d_stage = torch.empty_like(bufs[0])
+
+    def e2e_step(i):
+        sk.sk_frame_host(h_frames[i % len(h_frames)], cfg.M, h_SK, h_mask, d_stage, out.SK, out.mask,
+                         n_sigma=n_sigma, sk_mean=sk_mean, zero_flagged=False, workspace=ws, stream=stream)
+
+    e2e_step(0)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(Ke):
+        e2e_step(i)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s = float(te.item())
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    samples_per_step = frame_bytes * world
+    value = samples_per_step * K / (ms * 1e-3)
+    cells = cfg.B * cfg.F
+    out_bytes = cells * 5
+    flagged_bytes = int(flagged * frame_bytes) if args.zero else 0
+    alg_bytes = frame_bytes + out_bytes + flagged_bytes          # per launch (1 B/sample read)
+    peak, peak_src = peaks()
+    achieved = alg_bytes / (ms * 1e-3 / K) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8->u32/f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "N": cfg.E,
+                   "n_sigma": n_sigma, "sk_mean": sk_mean, "zero_flagged": bool(args.zero),
+                   "frame_bytes": frame_bytes, "flagged_fraction": flagged,
+                   "l2": f"rotating over {nbuf} distinct frames ({nbuf * frame_bytes >> 20} MiB > 126 MB L2)",
+                   "launch": "one CUDA graph of K sk_frame calls" if graph is not None else "K direct sk_frame calls",
+                   "parallelism": f"{world} independent replicas (no collective)"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": stored_traffic(cfg.name), "peak_source": peak_src,
+                     "frac_of_nominal_8000": achieved / 8000.0, "kernel": "sk_frame_kernel",
+                     "algorithmic_bytes_per_launch": alg_bytes},
+        "e2e": {"value": frame_bytes * world * Ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": frame_bytes,
+                "d2h_bytes_per_step": out_bytes, "steps": Ke, "api": "sk_frame_host (C ABI, pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "clocks": sampler.summary(),
+    }
+
+    if not args.no_cpu_baseline:
+        from oracle import sk_oracle
+        host = h_frames[0].numpy()
+        max_bytes = 100 * 1024 * 1024
+        blocks = max(1, min(cfg.B, max_bytes // (cfg.M * cfg.F * cfg.E)))
+        host = host[: blocks * cfg.M]
+        n, t0 = 0, time.perf_counter()
+        while True:
+            sk_oracle.frame(host, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean)
+            n += 1
+            if time.perf_counter() - t0 >= args.cpu_seconds:
+                break
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": host.size * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{n} passes over {blocks} of {cfg.B} blocks of {cfg.name} "
+                                          f"({host.size} samples each), {dt:.1f} s, single thread; "
+                                          f"host has {os.cpu_count()} cores"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

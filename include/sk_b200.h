@@ -1,0 +1,108 @@
+/* sk_b200.h — C ABI of the B200 spectral-kurtosis (SK) RFI detector.
+ *
+ * Implements the data-parallel hot path of arXiv 1808.10365 ("Spectral Kurtosis Based RFI
+ * Mitigation for CHIME"; citations are lines of /root/reference/PAPER.md):
+ *
+ *   a1-a3  unpack 4+4-bit samples, |x|^2, S1 = sum |x|^2, S2 = sum |x|^4 per M-sample block
+ *          (PAPER.md:45 Eq. 1, :77 Eq. 7, :278 for the 4+4-bit data)
+ *   a4-a6  SK~ = (M+1)/(M-1) * (S2bar/(M N) - 1),  S2bar = sum_i M^2 (S2)_i / (S1)_i^2
+ *          (PAPER.md:84-88 Eq. 9-11, :108-113 Eq. 14 — the estimator CHIME runs)
+ *   a7     flag cells outside sk_mean +- n_sigma * sqrt(4/(M N))   (PAPER.md:183, :119 Eq. 16, :284)
+ *   a8     optional excision of flagged cells
+ *
+ * Conventions common to every call
+ *   - Layout: data[T][F][E] uint8, E contiguous.  byte = (re+8)<<4 | (im+8), re, im in [-8, 7]
+ *     (nibble 0 decodes to -8; the encoded zero sample is 0x88).  A "cell" is one (block b,
+ *     frequency f): rows t = b*M .. (b+1)*M-1, each E contiguous bytes at stride F*E.
+ *     B = T/M blocks.  S1, S2: uint32 [B][F][E].  SK: float32 [B][F].  mask: uint8 [B][F].
+ *   - Pointers are DEVICE pointers owned by the caller unless the name starts with h_.
+ *     The library allocates no device memory, never synchronises the device (except
+ *     sk_frame_host, which waits for its own copies) and enqueues all work on `stream`
+ *     (a cudaStream_t cast to void*; NULL = the legacy default stream) before returning.
+ *   - Return value: 0 = enqueued; < 0 = argument error (SK_ERR_*), nothing was enqueued;
+ *     > 0 = a cudaError_t reported by a launch or copy.  No exceptions, no global state.
+ *   - Receiver selection ("total number of receivers"): `subset` is NULL or E
+ *     bytes on the device (non-zero = combine this input).  With subset == NULL the first
+ *     `first_n` inputs are combined (first_n = E for the whole array).  N is the number of
+ *     combined inputs; with a subset it is counted on the device.  An empty subset yields
+ *     SK = NaN and mask = 1 for every cell.
+ *   - A receiver whose S1 is 0 contributes the term M (its own SK^_i taken as 0), so an
+ *     all-0x88 cell gives SK = 0 exactly and re-running on excised data is NaN-free.
+ *   - Limits: 2 <= M <= 65536, T % M == 0, T, F, E >= 1, T*F*E < 2^40.
+ *     Any E and any alignment is accepted; E % 16 == 0 with a 16-byte-aligned `data` takes the
+ *     vector kernels, everything else a slower scalar kernel with identical results.
+ *   - Floating point: per-input terms and the sum over inputs are float64 in a fixed order
+ *     (deterministic run to run); SK is that value rounded to float32; the flag decision is
+ *     taken in float32: fabsf(SK - sk_mean) > (float)(n_sigma * sqrt(4.0/(M*N))), strict,
+ *     NaN => flagged.
+ */
+#ifndef SK_B200_H
+#define SK_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SK_OK                 0
+#define SK_ERR_NULL          -1   /* a required pointer is NULL */
+#define SK_ERR_SHAPE         -2   /* T, F, E, B out of range, or T % M != 0, or too large */
+#define SK_ERR_M             -3   /* M < 2 or M > 65536 */
+#define SK_ERR_N             -4   /* first_n == 0 or first_n > E (subset == NULL), or N == 0 */
+#define SK_ERR_PARAM         -5   /* n_sigma or sk_mean not finite, n_sigma < 0 */
+#define SK_ERR_WORKSPACE     -6   /* workspace NULL, misaligned (8 bytes) or too small */
+
+/* a1-a3 (Eq. 7).  Reads data[T][F][E]; writes S1, S2 [T/M][F][E] (exact integers). */
+int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                  uint32_t* S1, uint32_t* S2, void* stream);
+
+/* a4-a6 (PAPER.md:84-88 Eq. 9-11, :108-113 Eq. 14).  Reads S1, S2 [B][F][E]; writes SK [B][F]. */
+int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E,
+               uint32_t M, const uint8_t* subset, uint32_t first_n, float* SK, void* stream);
+
+/* a7 (variance PAPER.md:119 Eq. 16; centre sk_mean = 1 by Eq. 15 or the simulated
+ * null mean of PAPER.md:284).  Reads SK [B][F]; writes mask [B][F] (0/1). */
+int sk_flag(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, float n_sigma,
+            float sk_mean, uint8_t* mask, void* stream);
+
+/* Bytes of device workspace sk_frame needs for this shape (0 on a bad shape).  The workspace
+ * must be 8-byte aligned and ZERO-FILLED before its first use; every completed sk_frame call
+ * leaves it zero-filled again, so it can be reused by later calls on the same stream without
+ * clearing.  Do not share one workspace between calls that may run concurrently. */
+size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M);
+
+/* a1-a8 in one pass over HBM.  Writes SK and mask [T/M][F]; S1_opt / S2_opt [T/M][F][E] are
+ * written when non-NULL.  If zero_flagged != 0, every byte (all E inputs, all M rows) of each
+ * flagged cell is overwritten in place with 0x88 after the mask is known (the mask and SK are
+ * those of the data before excision); otherwise `data` is only read. */
+int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+             const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
+             int zero_flagged, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
+             void* workspace, size_t workspace_bytes, void* stream);
+
+/* End-to-end form with HOST buffers (pinned memory recommended): copies h_data to d_data,
+ * runs sk_frame there, copies SK and mask (and, if zero_flagged, the excised data) back, and
+ * waits for the copies.  d_data (T*F*E bytes), d_SK, d_mask, workspace are caller-owned device
+ * buffers; subset is a device pointer as above.  h_data is written only if zero_flagged. */
+int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                  const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
+                  int zero_flagged, float* h_SK, uint8_t* h_mask,
+                  uint8_t* d_data, float* d_SK, uint8_t* d_mask,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* Text for a return value of the calls above (static storage; never NULL). */
+const char* sk_strerror(int code);
+
+/* Library version: major*10000 + minor*100 + patch. */
+int sk_version(void);
+
+/* Number of kernels the library has launched in this process so far (for the bench's
+ * gpu_launches count; monotonically increasing, thread-safe). */
+unsigned long long sk_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SK_B200_H */

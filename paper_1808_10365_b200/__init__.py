@@ -1,0 +1,12 @@
+"""B200-native spectral-kurtosis (SK) RFI detector — the hot path of arXiv 1808.10365.
+
+The product is the C-ABI library built from csrc/ (declared in include/sk_b200.h); this package is
+its thin Python binding.  See DESIGN.md.
+"""
+from .binding import (SKError, SKResult, LIB_PATH, SYMBOLS, lib, sk_combine, sk_flag, sk_frame,
+                      sk_frame_host, sk_frame_workspace_bytes, sk_launch_count, sk_power_sums,
+                      sk_strerror, sk_version, workspace_for)
+
+__all__ = ["SKError", "SKResult", "LIB_PATH", "SYMBOLS", "lib", "sk_combine", "sk_flag", "sk_frame",
+           "sk_frame_host", "sk_frame_workspace_bytes", "sk_launch_count", "sk_power_sums",
+           "sk_strerror", "sk_version", "workspace_for"]

@@ -1,0 +1,210 @@
+"""Thin ctypes binding of libsk_b200.so (include/sk_b200.h): argument marshalling only.
+
+Every step of the SK path (arXiv 1808.10365: Eq. 7, 9-11, 14, flag, excision) runs in the CUDA
+kernels under csrc/.  PyTorch is used here for device memory and streams, nothing else.  There
+is no CPU fallback: a missing library or a non-CUDA tensor raises.
+"""
+import ctypes as C
+import os
+from typing import NamedTuple, Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
+
+SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
+           "sk_frame_host", "sk_strerror", "sk_version", "sk_launch_count")
+
+_lib = None
+
+
+class SKError(RuntimeError):
+    pass
+
+
+def lib() -> C.CDLL:
+    """Load the C-ABI library (built in-tree by `python -m paper_1808_10365_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise SKError(f"{LIB_PATH} is missing: build it with `python -m paper_1808_10365_b200.build` "
+                      "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    u32, vp, f32, i32, sz = C.c_uint32, C.c_void_p, C.c_float, C.c_int, C.c_size_t
+    L.sk_power_sums.argtypes = [vp, u32, u32, u32, u32, vp, vp, vp]
+    L.sk_combine.argtypes = [vp, vp, u32, u32, u32, u32, vp, u32, vp, vp]
+    L.sk_flag.argtypes = [vp, u32, u32, u32, u32, f32, f32, vp, vp]
+    L.sk_frame_workspace_bytes.argtypes = [u32, u32, u32, u32]
+    L.sk_frame_workspace_bytes.restype = sz
+    L.sk_frame.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_frame_host.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_strerror.argtypes = [i32]
+    L.sk_strerror.restype = C.c_char_p
+    L.sk_version.restype = i32
+    L.sk_launch_count.restype = C.c_ulonglong
+    for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host"):
+        getattr(L, name).restype = i32
+    _lib = L
+    return L
+
+
+def sk_strerror(code: int) -> str:
+    return lib().sk_strerror(int(code)).decode()
+
+
+def sk_version() -> int:
+    return int(lib().sk_version())
+
+
+def sk_launch_count() -> int:
+    return int(lib().sk_launch_count())
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise SKError(f"{what} failed ({rc}): {sk_strerror(rc)}")
+
+
+def _dev(t: torch.Tensor, dtype, what: str) -> torch.Tensor:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise SKError(f"{what} must be a CUDA tensor (there is no CPU path)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise SKError(f"{what} must be a contiguous {dtype} tensor")
+    return t
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _subset(subset, E, device):
+    if subset is None:
+        return None
+    s = torch.as_tensor(subset)
+    s = (s != 0).to(torch.uint8).to(device).contiguous()
+    if s.shape != (E,):
+        raise SKError("subset must have E entries")
+    return s
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else t.data_ptr()
+
+
+class SKResult(NamedTuple):
+    SK: torch.Tensor
+    mask: torch.Tensor
+    S1: Optional[torch.Tensor]
+    S2: Optional[torch.Tensor]
+
+
+_ws_cache = {}
+
+
+def sk_frame_workspace_bytes(T: int, F: int, E: int, M: int) -> int:
+    return int(lib().sk_frame_workspace_bytes(T, F, E, M))
+
+
+def workspace_for(T, F, E, M, device, stream_id=0) -> torch.Tensor:
+    """A zero-filled device workspace for sk_frame, cached per (device, stream, size).  The library
+    leaves a workspace zero-filled after every call, so it is cleared only when created."""
+    n = sk_frame_workspace_bytes(T, F, E, M)
+    if n == 0:
+        raise SKError("bad shape for sk_frame")
+    key = (str(device), stream_id, n)
+    ws = _ws_cache.get(key)
+    if ws is None:
+        ws = torch.zeros((n + 7) // 8, dtype=torch.int64, device=device)
+        _ws_cache[key] = ws
+    return ws
+
+
+def sk_power_sums(data: torch.Tensor, M: int, stream=None):
+    """PAPER.md:77 Eq. 7.  data uint8 [T][F][E] (CUDA) -> S1, S2 uint32 [T/M][F][E]."""
+    _dev(data, torch.uint8, "data")
+    T, F, E = data.shape
+    B = T // M if M else 0
+    S1 = torch.empty((B, F, E), dtype=torch.uint32, device=data.device)
+    S2 = torch.empty_like(S1)
+    _check(lib().sk_power_sums(data.data_ptr(), T, F, E, M, S1.data_ptr(), S2.data_ptr(), _stream(stream)),
+           "sk_power_sums")
+    return S1, S2
+
+
+def sk_combine(S1: torch.Tensor, S2: torch.Tensor, M: int, subset=None, first_n=None, stream=None):
+    """PAPER.md:84-88 Eq. 9-11, :108-113 Eq. 14.  S1, S2 uint32 [B][F][E] -> SK float32 [B][F]."""
+    _dev(S1, torch.uint32, "S1")
+    _dev(S2, torch.uint32, "S2")
+    B, F, E = S1.shape
+    sub = _subset(subset, E, S1.device)
+    if sub is None and first_n is None:
+        first_n = E
+    SK = torch.empty((B, F), dtype=torch.float32, device=S1.device)
+    _check(lib().sk_combine(S1.data_ptr(), S2.data_ptr(), B, F, E, M, _ptr(sub), int(first_n or 0),
+                            SK.data_ptr(), _stream(stream)), "sk_combine")
+    return SK
+
+
+def sk_flag(SK: torch.Tensor, M: int, N: int, n_sigma: float, sk_mean: float = 1.0, stream=None):
+    """PAPER.md:183 / :119 Eq. 16.  SK float32 [B][F] -> mask uint8 [B][F]."""
+    _dev(SK, torch.float32, "SK")
+    B, F = SK.shape
+    mask = torch.empty((B, F), dtype=torch.uint8, device=SK.device)
+    _check(lib().sk_flag(SK.data_ptr(), B, F, M, N, n_sigma, sk_mean, mask.data_ptr(), _stream(stream)),
+           "sk_flag")
+    return mask
+
+
+def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: float = 3.0,
+             sk_mean: float = 1.0, zero_flagged: bool = False, want_sums: bool = False,
+             out: Optional[SKResult] = None, workspace: Optional[torch.Tensor] = None,
+             stream=None) -> SKResult:
+    """The fused path (one pass over HBM).  `data` is modified in place only if zero_flagged."""
+    _dev(data, torch.uint8, "data")
+    T, F, E = data.shape
+    B = T // M if M else 0
+    dev = data.device
+    sub = subset if (isinstance(subset, torch.Tensor) and subset.is_cuda and subset.dtype == torch.uint8
+                     and subset.is_contiguous() and subset.shape == (E,)) else _subset(subset, E, dev)
+    if sub is None and first_n is None:
+        first_n = E
+    st = _stream(stream)
+    if out is None:
+        SK = torch.empty((B, F), dtype=torch.float32, device=dev)
+        mask = torch.empty((B, F), dtype=torch.uint8, device=dev)
+        S1 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
+        S2 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
+        out = SKResult(SK, mask, S1, S2)
+    if workspace is None:
+        workspace = workspace_for(T, F, E, M, dev, st)
+    _check(lib().sk_frame(data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
+                          int(bool(zero_flagged)), out.SK.data_ptr(), out.mask.data_ptr(),
+                          _ptr(out.S1), _ptr(out.S2), workspace.data_ptr(),
+                          workspace.numel() * workspace.element_size(), st), "sk_frame")
+    return out
+
+
+def sk_frame_host(h_data: torch.Tensor, M: int, h_SK: torch.Tensor, h_mask: torch.Tensor,
+                  d_data: torch.Tensor, d_SK: torch.Tensor, d_mask: torch.Tensor, subset=None,
+                  first_n=None, n_sigma: float = 3.0, sk_mean: float = 1.0, zero_flagged: bool = False,
+                  workspace: Optional[torch.Tensor] = None, stream=None):
+    """End-to-end form: host buffers in and out (pinned recommended), copies inside the call."""
+    if h_data.is_cuda or h_SK.is_cuda or h_mask.is_cuda:
+        raise SKError("h_* tensors must live in host memory")
+    T, F, E = h_data.shape
+    _dev(d_data, torch.uint8, "d_data")
+    sub = _subset(subset, E, d_data.device)
+    if sub is None and first_n is None:
+        first_n = E
+    st = _stream(stream)
+    if workspace is None:
+        workspace = workspace_for(T, F, E, M, d_data.device, st)
+    _check(lib().sk_frame_host(h_data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma,
+                               sk_mean, int(bool(zero_flagged)), h_SK.data_ptr(), h_mask.data_ptr(),
+                               d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
+                               workspace.numel() * workspace.element_size(), st), "sk_frame_host")
+    return h_SK, h_mask

@@ -1,0 +1,259 @@
+// sk_api.cu — the C ABI of include/sk_b200.h: argument checks, shape -> kernel choice, launches.
+// Nothing here allocates device memory or synchronises (sk_frame_host waits for its own copies).
+#include <atomic>
+#include <cmath>
+#include <cstdint>
+
+#include "../../include/sk_b200.h"
+#include "sk_kernels.cuh"
+
+namespace {
+
+std::atomic<unsigned long long> g_launches{0};
+
+inline int launch_status() {
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SK_OK : (int)e;
+}
+
+// Lanes per row for the vector path: a function of E only, so that sk_combine and sk_frame
+// split a cell into the same units and add the float64 terms in the same order.
+inline int lanes_per_row(uint32_t E) {
+    const uint32_t vecs = E / 16;            // 128-bit vectors per row
+    int L = 16;                              // 256-byte slabs for wide arrays
+    while (L > 1 && (uint32_t)L > vecs) L >>= 1;
+    return L;
+}
+
+inline bool vector_ok(const void* data, uint32_t E) {
+    return E % 16 == 0 && (reinterpret_cast<uintptr_t>(data) & 15u) == 0;
+}
+
+int check_shape(uint32_t T, uint32_t F, uint32_t E, uint32_t M) {
+    if (M < 2 || M > 65536) return SK_ERR_M;
+    if (T == 0 || F == 0 || E == 0 || T % M != 0) return SK_ERR_SHAPE;
+    const unsigned long long total = (unsigned long long)T * F * E;
+    if (total >= (1ull << 40)) return SK_ERR_SHAPE;
+    if ((unsigned long long)(T / M) * F >= (1ull << 31)) return SK_ERR_SHAPE;
+    if (E > (1u << 20)) return SK_ERR_SHAPE;
+    return SK_OK;
+}
+
+struct Plan {
+    bool vec;
+    int L;
+    uint32_t slabs;       // launched slabs per cell
+    bool wide;            // AccWide usable (samples per lane <= 511)
+};
+
+Plan make_plan(const void* data, uint32_t E, uint32_t M, const uint8_t* subset, uint32_t first_n,
+               bool need_all_inputs) {
+    Plan pl{};
+    pl.vec = vector_ok(data, E);
+    pl.L = lanes_per_row(E);
+    const uint32_t W = 16u * pl.L;
+    uint32_t cover = E;
+    if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
+    pl.slabs = (cover + W - 1) / W;
+    const uint32_t RPW = 32u / pl.L;
+    const uint32_t iters = (M + RPW - 1) / RPW;
+    const uint32_t padded = (iters + sk::kUnroll - 1) / sk::kUnroll * sk::kUnroll;
+    pl.wide = padded <= sk::AccWide::kMaxSamples;
+    return pl;
+}
+
+template <class Acc>
+void launch_vec_L(int L, const sk::FrameParams& p, cudaStream_t st) {
+    const unsigned grid = (p.nunits + sk::kWarpsPerCta - 1) / sk::kWarpsPerCta;
+    const unsigned block = sk::kWarpsPerCta * 32;
+    switch (L) {
+        case 16: sk::sk_frame_kernel<16, Acc><<<grid, block, 0, st>>>(p); break;
+        case 8:  sk::sk_frame_kernel<8, Acc><<<grid, block, 0, st>>>(p); break;
+        case 4:  sk::sk_frame_kernel<4, Acc><<<grid, block, 0, st>>>(p); break;
+        case 2:  sk::sk_frame_kernel<2, Acc><<<grid, block, 0, st>>>(p); break;
+        default: sk::sk_frame_kernel<1, Acc><<<grid, block, 0, st>>>(p); break;
+    }
+    ++g_launches;
+}
+
+int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
+    const uint32_t cells = p.B * p.F;
+    if (pl.vec) {
+        p.slabs = pl.slabs;
+        p.nunits = cells * pl.slabs;
+        if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
+        else         launch_vec_L<sk::AccPlain>(pl.L, p, st);
+    } else {
+        sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);
+        ++g_launches;
+    }
+    return launch_status();
+}
+
+size_t workspace_bytes(uint32_t cells, uint32_t slabs_max) {
+    return (size_t)cells * slabs_max * sizeof(double) + (size_t)cells * sizeof(uint32_t);
+}
+
+}  // namespace
+
+extern "C" {
+
+int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                  uint32_t* S1, uint32_t* S2, void* stream) {
+    if (!data || !S1 || !S2) return SK_ERR_NULL;
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    Plan pl = make_plan(data, E, M, nullptr, E, true);
+    if ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) pl.vec = false;
+    sk::FrameParams p{};
+    p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
+    p.first_n = E;
+    p.S1out = S1; p.S2out = S2;
+    return launch_cells(pl, p, (cudaStream_t)stream);
+}
+
+size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M) {
+    if (check_shape(T, F, E, M)) return 0;
+    const uint32_t cells = (T / M) * F;
+    const int L = lanes_per_row(E);
+    const uint32_t slabs = (E + 16u * L - 1) / (16u * L);
+    return workspace_bytes(cells, slabs);
+}
+
+static int frame_impl(const uint8_t* data, uint32_t T,
+                      uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset, uint32_t first_n,
+                      float n_sigma, float sk_mean, float* SK, uint8_t* mask, uint32_t* S1o,
+                      uint32_t* S2o, void* workspace, size_t workspace_bytes_given, cudaStream_t st) {
+    if (!SK) return SK_ERR_NULL;
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
+    if (mask && (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0)) return SK_ERR_PARAM;
+    if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
+    Plan pl = make_plan(data, E, M, subset, first_n, S1o != nullptr);
+    if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
+    sk::FrameParams p{};
+    p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
+    p.subset = subset; p.first_n = subset ? 0 : first_n;
+    p.n_sigma = n_sigma; p.sk_mean = sk_mean;
+    p.SK = SK; p.mask = mask; p.S1out = S1o; p.S2out = S2o;
+    if (pl.vec) {
+        const uint32_t cells = p.B * F;
+        const size_t need = workspace_bytes(cells, pl.slabs);
+        if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) || workspace_bytes_given < need)
+            return SK_ERR_WORKSPACE;
+        p.partial = static_cast<double*>(workspace);
+        // counters sit after the largest possible partial array, so their place does not depend
+        // on first_n and a workspace stays clean across calls with different receiver subsets
+        const int L = pl.L;
+        const uint32_t slabs_max = (E + 16u * L - 1) / (16u * L);
+        if (workspace_bytes_given < workspace_bytes(cells, slabs_max)) return SK_ERR_WORKSPACE;
+        p.counter = reinterpret_cast<uint32_t*>(static_cast<double*>(workspace) + (size_t)cells * slabs_max);
+    }
+    return launch_cells(pl, p, st);
+}
+
+int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
+               const uint8_t* subset, uint32_t first_n, float* SK, void* stream) {
+    if (!S1 || !S2 || !SK) return SK_ERR_NULL;
+    if (B == 0 || (unsigned long long)B * M > 0xFFFFFFFFull) return SK_ERR_SHAPE;
+    if (int rc = check_shape(B * M, F, E, M)) return rc;
+    if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
+    cudaStream_t st = (cudaStream_t)stream;
+    sk::FrameParams p{};
+    p.T = B * M; p.F = F; p.E = E; p.M = M; p.B = B;
+    p.subset = subset; p.first_n = subset ? 0 : first_n;
+    p.SK = SK; p.S1in = S1; p.S2in = S2;
+    const uint32_t cells = B * F;
+    const bool vec = E % 16 == 0 &&
+                     ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) == 0;
+    if (vec) {
+        const int L = lanes_per_row(E);
+        p.slabs = (E + 16u * L - 1) / (16u * L);
+        p.nunits = cells * p.slabs;
+        const size_t smem = (size_t)p.slabs * sizeof(double);
+        if (smem > 48 * 1024) return SK_ERR_SHAPE;
+        const unsigned block = sk::kWarpsPerCta * 32;
+        switch (L) {
+            case 16: sk::sk_combine_kernel<16><<<cells, block, smem, st>>>(p); break;
+            case 8:  sk::sk_combine_kernel<8><<<cells, block, smem, st>>>(p); break;
+            case 4:  sk::sk_combine_kernel<4><<<cells, block, smem, st>>>(p); break;
+            case 2:  sk::sk_combine_kernel<2><<<cells, block, smem, st>>>(p); break;
+            default: sk::sk_combine_kernel<1><<<cells, block, smem, st>>>(p); break;
+        }
+    } else {
+        sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);
+    }
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_flag(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, float n_sigma,
+            float sk_mean, uint8_t* mask, void* stream) {
+    if (!SK || !mask) return SK_ERR_NULL;
+    if (M < 2 || M > 65536) return SK_ERR_M;
+    if (B == 0 || F == 0 || (unsigned long long)B * F >= (1ull << 31)) return SK_ERR_SHAPE;
+    if (N == 0) return SK_ERR_N;
+    if (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0) return SK_ERR_PARAM;
+    const size_t cells = (size_t)B * F;
+    const float thr = sk::flag_threshold(n_sigma, (double)M, (double)N);
+    sk::sk_flag_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, (cudaStream_t)stream>>>(SK, mask, cells,
+                                                                                         sk_mean, thr);
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
+             uint32_t first_n, float n_sigma, float sk_mean, int zero_flagged, float* SK, uint8_t* mask,
+             uint32_t* S1_opt, uint32_t* S2_opt, void* workspace, size_t workspace_bytes_given,
+             void* stream) {
+    if (!data || !SK || !mask) return SK_ERR_NULL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = frame_impl(data, T, F, E, M, subset, first_n, n_sigma, sk_mean, SK, mask,
+                        S1_opt, S2_opt, workspace, workspace_bytes_given, st);
+    if (rc != SK_OK || !zero_flagged) return rc;
+    const uint32_t cells = (T / M) * F;
+    const dim3 grid(cells, (M + sk::kExciseRows - 1) / sk::kExciseRows);
+    if (vector_ok(data, E)) sk::sk_excise_kernel<true><<<grid, 256, 0, st>>>(data, mask, F, E, M);
+    else                    sk::sk_excise_kernel<false><<<grid, 256, 0, st>>>(data, mask, F, E, M);
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
+                  uint32_t first_n, float n_sigma, float sk_mean, int zero_flagged, float* h_SK,
+                  uint8_t* h_mask, uint8_t* d_data, float* d_SK, uint8_t* d_mask, void* workspace,
+                  size_t workspace_bytes_given, void* stream) {
+    if (!h_data || !h_SK || !h_mask || !d_data || !d_SK || !d_mask) return SK_ERR_NULL;
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)T * F * E, cells = (size_t)(T / M) * F;
+    cudaError_t e = cudaMemcpyAsync(d_data, h_data, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return (int)e;
+    const int rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, zero_flagged, d_SK,
+                            d_mask, nullptr, nullptr, workspace, workspace_bytes_given, stream);
+    if (rc != SK_OK) return rc;
+    e = cudaMemcpyAsync(h_SK, d_SK, cells * sizeof(float), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_mask, d_mask, cells, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && zero_flagged)
+        e = cudaMemcpyAsync(h_data, d_data, bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? SK_OK : (int)e;
+}
+
+const char* sk_strerror(int code) {
+    switch (code) {
+        case SK_OK: return "ok";
+        case SK_ERR_NULL: return "a required pointer is NULL";
+        case SK_ERR_SHAPE: return "bad shape: T, F, E must be >= 1, T % M == 0, T*F*E < 2^40";
+        case SK_ERR_M: return "M must be in [2, 65536]";
+        case SK_ERR_N: return "receiver count N must be in [1, E]";
+        case SK_ERR_PARAM: return "n_sigma and sk_mean must be finite, n_sigma >= 0";
+        case SK_ERR_WORKSPACE: return "workspace is NULL, misaligned or smaller than sk_frame_workspace_bytes()";
+        default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
+    }
+}
+
+int sk_version(void) { return 100; }
+
+unsigned long long sk_launch_count(void) { return g_launches.load(); }
+
+}  // extern "C"

@@ -1,0 +1,130 @@
+// sk_device.cuh — device-side building blocks of the SK hot path (sm_100a).
+//
+// Steps (equations of arXiv 1808.10365, lines of PAPER.md):
+//   a1 unpack 4+4-bit offset samples      a2 |x|^2
+//   a3 S1 = sum |x|^2, S2 = sum |x|^4 (Eq. 7)
+//   a4 term_e = M^2 S2_e / S1_e^2 (Eq. 9, 11)
+// This file shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace sk {
+
+// ---------------------------------------------------------------------------------- loads
+// Streaming 128-bit load: read-only path, do not allocate in L1 (every byte is used once).
+__device__ __forceinline__ uint4 ldg_stream(const uint8_t* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+// ------------------------------------------------------------------------- a1 + a2, packed
+// One 32-bit word holds 4 samples: byte = (re+8)<<4 | (im+8).
+//   hi(w) = (w & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*re   (one LOP3)
+//   lo(w) = ((w<<4) & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*im (SHF + LOP3)
+// Flipping the top bit of the offset nibble turns it into two's complement, and leaving it in
+// the high nibble of its byte sign-extends it for free (scaled by 16).  Nibble 0 -> -128 = 16*(-8).
+__device__ __forceinline__ uint32_t re16(uint32_t w) { return (w & 0xF0F0F0F0u) ^ 0x80808080u; }
+__device__ __forceinline__ uint32_t im16(uint32_t w) { return ((w << 4) & 0xF0F0F0F0u) ^ 0x80808080u; }
+
+// Sample k of the word: C = [16re_k, 16im_k, 16re_k, 16im_k] (one PRMT), then one DP4A gives
+// C.C + c0 = 512 |x_k|^2 + c0  (|x|^2 <= 128, so 512|x|^2 <= 2^16).
+template <int K>
+__device__ __forceinline__ uint32_t power512(uint32_t r16, uint32_t i16, uint32_t c0) {
+    constexpr uint32_t sel = (uint32_t)K | ((4u + K) << 4) | ((uint32_t)K << 8) | ((4u + K) << 12);
+    const uint32_t c = __byte_perm(r16, i16, sel);
+    return (uint32_t)__dp4a((int)c, (int)c, (int)c0);
+}
+
+// ------------------------------------------------------------------------------ a3 variants
+// Accumulator for one input.  Two exact strategies with the same interface:
+//
+// AccPlain: S1 += p; S2 += p*p in two 32-bit registers (shift, add, IMAD per sample).
+//
+// AccWide : ONE 64-bit multiply-add per sample.  With q = 512 p + 2^31 (the 2^31 comes free as the
+//   DP4A addend), q*q = 2^18 p^2 + 2^41 p + 2^62, so a 64-bit accumulator collects
+//   sum p^2 in bits 18..40 and sum p in bits 41..61; the constant n*2^62 (n = samples added) wraps
+//   mod 2^64 and is removed at read-out.  Exact while sum p^2 < 2^23, i.e. n <= 511 samples
+//   (p^2 <= 2^14) — callers flush at most every 256.
+struct AccPlain {
+    uint32_t s1, s2;
+    static constexpr uint32_t kAddend = 0u;
+    __device__ __forceinline__ void reset() { s1 = 0; s2 = 0; }
+    __device__ __forceinline__ void add(uint32_t q) { const uint32_t p = q >> 9; s1 += p; s2 += p * p; }
+    __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const { S1 = s1; S2 = s2; }
+};
+
+struct AccWide {
+    unsigned long long a;
+    static constexpr uint32_t kAddend = 0x80000000u;
+    static constexpr uint32_t kMaxSamples = 511;
+    __device__ __forceinline__ void reset() { a = 0ull; }
+    __device__ __forceinline__ void add(uint32_t q) { a += (unsigned long long)q * q; }
+    __device__ __forceinline__ void read(uint32_t n, uint32_t& S1, uint32_t& S2) const {
+        const unsigned long long v = a - ((unsigned long long)(n & 3u) << 62);
+        S1 = (uint32_t)(v >> 41);
+        S2 = (uint32_t)((v & ((1ull << 41) - 1ull)) >> 18);
+    }
+};
+
+// Add the 16 samples of one 128-bit load to 16 accumulators.
+template <class Acc>
+__device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v) {
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t r = re16(w[i]), m = im16(w[i]);
+        acc[4 * i + 0].add(power512<0>(r, m, Acc::kAddend));
+        acc[4 * i + 1].add(power512<1>(r, m, Acc::kAddend));
+        acc[4 * i + 2].add(power512<2>(r, m, Acc::kAddend));
+        acc[4 * i + 3].add(power512<3>(r, m, Acc::kAddend));
+    }
+}
+
+// Scalar a1-a2 for the fallback kernel.
+__device__ __forceinline__ uint32_t power_scalar(uint8_t byte) {
+    const int re = (int)(byte >> 4) - 8, im = (int)(byte & 15) - 8;
+    return (uint32_t)(re * re + im * im);
+}
+
+// ------------------------------------------------------------------------------------- a4
+// term = M^2 S2 / S1^2 in float64, every operation individually rounded (no FMA contraction);
+// a receiver with S1 == 0 contributes M (header: "A receiver whose S1 is 0 ...").
+__device__ __forceinline__ double eq11_term(double M, uint32_t S1, uint32_t S2) {
+    if (S1 == 0u) return M;
+    const double s1 = (double)S1, s2 = (double)S2;
+    return __ddiv_rn(__dmul_rn(__dmul_rn(M, M), s2), __dmul_rn(s1, s1));
+}
+
+// a6: SK~ = (M+1)/(M-1) * (S2bar/(M N) - 1)  (Eq. 14, second line), then float32.
+__device__ __forceinline__ float eq14_sk(double S2bar, double M, double N) {
+    const double a = __ddiv_rn(__dadd_rn(M, 1.0), __dsub_rn(M, 1.0));
+    const double c = __ddiv_rn(S2bar, __dmul_rn(M, N));
+    return __double2float_rn(__dmul_rn(a, __dsub_rn(c, 1.0)));
+}
+
+// a7: flagged iff fabsf(SK - sk_mean) > thr in float32, strict; NaN => flagged.
+__device__ __forceinline__ uint8_t flag_decision(float SK, float sk_mean, float thr) {
+    const float dev = fabsf(__fsub_rn(SK, sk_mean));
+    return (dev > thr || dev != dev) ? 1 : 0;
+}
+
+// thr = (float)(n_sigma * sqrt(4/(M N))) — float64 inside, as the header states.
+__host__ __device__ __forceinline__ float flag_threshold(float n_sigma, double M, double N) {
+#ifdef __CUDA_ARCH__
+    return __double2float_rn(__dmul_rn((double)n_sigma, __dsqrt_rn(__ddiv_rn(4.0, __dmul_rn(M, N)))));
+#else
+    return (float)((double)n_sigma * sqrt(4.0 / (M * N)));
+#endif
+}
+
+__device__ __forceinline__ double warp_sum_fixed(double x) {
+    // fixed butterfly: the same association order on every run
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = __dadd_rn(x, __shfl_xor_sync(0xffffffffu, x, o));
+    return x;
+}
+
+}  // namespace sk

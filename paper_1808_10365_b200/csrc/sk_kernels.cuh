@@ -1,0 +1,288 @@
+// sk_kernels.cuh — the kernels of the SK hot path (sm_100a).  See sk_device.cuh for the arithmetic.
+//
+// Work decomposition (vector path, E % 16 == 0, 16-byte aligned data):
+//   unit  = one (cell, slab): M rows x W = 16*L contiguous inputs, handled by ONE warp.
+//   lane  = (row group r0 = lane / L, column cl = lane % L): 16 inputs e0..e0+15 of every
+//           RPW-th row (RPW = 32/L rows are covered by one warp-wide 128-bit load).
+//   After the row loop the RPW row groups are summed with shuffles (integers: exact), each lane
+//   evaluates Eq. 11's term for its share of the 16 inputs in float64, the warp adds them with a
+//   fixed butterfly, and the unit's partial S2bar goes to the workspace.  The last unit of a cell
+//   to arrive (one atomic counter per cell) adds the partials in ascending slab order, evaluates
+//   Eq. 14, rounds to float32, takes the flag decision, and resets the counter.
+//   The order of every floating-point sum is fixed, so results are bit-reproducible.
+#pragma once
+#include "sk_device.cuh"
+
+namespace sk {
+
+struct FrameParams {
+    const uint8_t* data;      // [T][F][E]
+    uint32_t T, F, E, M, B;
+    const uint8_t* subset;    // E bytes or nullptr
+    uint32_t first_n;         // used when subset == nullptr
+    float n_sigma, sk_mean;
+    float* SK;                // [B][F] or nullptr (power-sums only)
+    uint8_t* mask;            // [B][F] or nullptr
+    uint32_t* S1out;          // [B][F][E] or nullptr
+    uint32_t* S2out;
+    const uint32_t* S1in;     // combine: read sums instead of data
+    const uint32_t* S2in;
+    double* partial;          // workspace: [cells][slabs]
+    uint32_t* counter;        // workspace: [cells], zero on entry, zero on exit
+    uint32_t slabs;           // units per cell that are launched
+    uint32_t nunits;          // cells * slabs
+};
+
+constexpr int kWarpsPerCta = 4;
+constexpr int kUnroll = 8;     // 128-bit loads in flight per lane
+
+// Number of combined receivers N: first_n, or the count of non-zero subset bytes (whole warp).
+__device__ __forceinline__ uint32_t count_receivers(const FrameParams& p, int lane) {
+    if (!p.subset) return p.first_n;
+    uint32_t n = 0;
+    for (uint32_t e = lane; e < p.E; e += 32) n += (__ldg(p.subset + e) != 0);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+    return n;
+}
+
+__device__ __forceinline__ bool selected(const FrameParams& p, uint32_t e) {
+    return p.subset ? (__ldg(p.subset + e) != 0) : (e < p.first_n);
+}
+
+// a4 + a5 (within a unit): the unit's share of S2bar, identical on all lanes on return.
+// Called by the fused kernel and by the combine kernel, so both add in the same order.
+template <int L>
+__device__ __forceinline__ double unit_partial(const FrameParams& p, int lane, bool active, uint32_t e0,
+                                               const uint32_t (&S1)[16], const uint32_t (&S2)[16]) {
+    constexpr int RPW = 32 / L;
+    const int r0 = lane / L;
+    const double Md = (double)p.M;
+    double part = 0.0;
+    if (active) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            if ((k % RPW) == r0 && selected(p, e0 + k))      // share the 16 inputs among row groups
+                part = __dadd_rn(part, eq11_term(Md, S1[k], S2[k]));
+        }
+    }
+    return warp_sum_fixed(part);
+}
+
+// a5 (across units, ascending slab order) + a6 + a7 for one cell; whole warp calls, lane 0 writes.
+__device__ __forceinline__ void finalize_cell(const FrameParams& p, uint32_t cell, int lane,
+                                              const volatile double* partials) {
+    const uint32_t N = count_receivers(p, lane);
+    if (lane == 0) {
+        const double Md = (double)p.M;
+        double S2bar = 0.0;
+        for (uint32_t s = 0; s < p.slabs; ++s) S2bar = __dadd_rn(S2bar, partials[s]);
+        const float sk = eq14_sk(S2bar, Md, (double)N);
+        p.SK[cell] = sk;
+        if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, (double)N));
+    }
+}
+
+// Fused kernel: publish the unit's partial; the last unit of the cell to arrive finalizes it.
+__device__ __forceinline__ void publish_and_finalize(const FrameParams& p, uint32_t cell, uint32_t slab,
+                                                     int lane, double part) {
+    uint32_t last = 0;
+    if (lane == 0) {
+        p.partial[(size_t)cell * p.slabs + slab] = part;
+        __threadfence();
+        last = (atomicAdd(p.counter + cell, 1u) == p.slabs - 1u);
+    }
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (!last) return;
+    __threadfence();
+    finalize_cell(p, cell, lane, p.partial + (size_t)cell * p.slabs);
+    if (lane == 0) p.counter[cell] = 0u;                     // leave the workspace clean
+}
+
+// --------------------------------------------------------------------------- fused a1..a7
+template <int L, class Acc>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+sk_frame_kernel(const FrameParams p) {
+    constexpr int RPW = 32 / L;
+    const int lane = threadIdx.x & 31;
+    const uint32_t unit = blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5);
+    if (unit >= p.nunits) return;
+    const uint32_t slab = unit % p.slabs, cell = unit / p.slabs;
+    const uint32_t b = cell / p.F, f = cell % p.F;
+    const int cl = lane % L, r0 = lane / L;
+    const uint32_t e0 = (slab * L + cl) * 16u;
+    const bool active = e0 < p.E;
+
+    uint32_t S1[16], S2[16];
+    {
+        Acc acc[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) acc[k].reset();
+        const size_t rstride = (size_t)p.F * p.E;
+        const uint8_t* base = p.data + ((size_t)b * p.M * p.F + f) * p.E + e0;
+        uint32_t n = 0;
+        if (active) {
+            for (uint32_t j = r0; j < p.M; j += RPW * kUnroll) {
+                uint4 v[kUnroll];
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) {
+                    const uint32_t jj = j + u * RPW;
+                    v[u] = (jj < p.M) ? ldg_stream(base + (size_t)jj * rstride)
+                                      : make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
+                }
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) accumulate16(acc, v[u]);
+                n += kUnroll;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k) acc[k].read(n, S1[k], S2[k]);
+        // sum the RPW row groups: afterwards every lane of column cl holds the cell totals
+#pragma unroll
+        for (int o = L; o < 32; o <<= 1) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                S1[k] += __shfl_xor_sync(0xffffffffu, S1[k], o);
+                S2[k] += __shfl_xor_sync(0xffffffffu, S2[k], o);
+            }
+        }
+        if (p.S1out && active && r0 == 0) {
+            uint4* o1 = reinterpret_cast<uint4*>(p.S1out + (size_t)cell * p.E + e0);
+            uint4* o2 = reinterpret_cast<uint4*>(p.S2out + (size_t)cell * p.E + e0);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                o1[i] = make_uint4(S1[4 * i], S1[4 * i + 1], S1[4 * i + 2], S1[4 * i + 3]);
+                o2[i] = make_uint4(S2[4 * i], S2[4 * i + 1], S2[4 * i + 2], S2[4 * i + 3]);
+            }
+        }
+    }
+    if (p.SK) publish_and_finalize(p, cell, slab, lane, unit_partial<L>(p, lane, active, e0, S1, S2));
+}
+
+// ------------------------------------------------------------------ a4..a6 from stored sums
+// One CTA per cell; its warps walk the cell's slabs with the same lane mapping as the fused
+// kernel, keep the per-slab partials in shared memory, and warp 0 finalizes: bit-identical SK.
+template <int L>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+sk_combine_kernel(const FrameParams p) {
+    extern __shared__ double partials[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t cell = blockIdx.x;
+    const int cl = lane % L;
+    for (uint32_t slab = warp; slab < p.slabs; slab += kWarpsPerCta) {
+        const uint32_t e0 = (slab * L + cl) * 16u;
+        const bool active = e0 < p.E;
+        uint32_t S1[16], S2[16];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            uint4 a = make_uint4(0, 0, 0, 0), c = a;
+            if (active) {
+                a = __ldg(reinterpret_cast<const uint4*>(p.S1in + (size_t)cell * p.E + e0) + i);
+                c = __ldg(reinterpret_cast<const uint4*>(p.S2in + (size_t)cell * p.E + e0) + i);
+            }
+            S1[4 * i] = a.x; S1[4 * i + 1] = a.y; S1[4 * i + 2] = a.z; S1[4 * i + 3] = a.w;
+            S2[4 * i] = c.x; S2[4 * i + 1] = c.y; S2[4 * i + 2] = c.z; S2[4 * i + 3] = c.w;
+        }
+        const double part = unit_partial<L>(p, lane, active, e0, S1, S2);
+        if (lane == 0) partials[slab] = part;
+    }
+    __syncthreads();
+    if (warp == 0) finalize_cell(p, cell, lane, partials);
+}
+
+// ------------------------------------------------------------- scalar fallback (any E, alignment)
+// One CTA per cell; thread t owns inputs t, t+256, ...; float64 terms are added per thread in
+// ascending e, then across threads with a fixed shared-memory tree.
+constexpr int kScalarThreads = 256;
+
+__global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const FrameParams p) {
+    __shared__ double red[kScalarThreads];
+    __shared__ uint32_t cnt[kScalarThreads];
+    const uint32_t cell = blockIdx.x;
+    const uint32_t b = cell / p.F, f = cell % p.F;
+    const double Md = (double)p.M;
+    double part = 0.0;
+    uint32_t nsel = 0;
+    for (uint32_t e = threadIdx.x; e < p.E; e += kScalarThreads) {
+        uint32_t s1 = 0, s2 = 0;
+        if (p.S1in) {
+            s1 = p.S1in[(size_t)cell * p.E + e];
+            s2 = p.S2in[(size_t)cell * p.E + e];
+        } else {
+            const uint8_t* q = p.data + ((size_t)b * p.M * p.F + f) * p.E + e;
+            const size_t rstride = (size_t)p.F * p.E;
+            for (uint32_t j = 0; j < p.M; ++j) {
+                const uint32_t pw = power_scalar(q[(size_t)j * rstride]);
+                s1 += pw;
+                s2 += pw * pw;
+            }
+            if (p.S1out) {
+                p.S1out[(size_t)cell * p.E + e] = s1;
+                p.S2out[(size_t)cell * p.E + e] = s2;
+            }
+        }
+        if (p.SK && selected(p, e)) {
+            part = __dadd_rn(part, eq11_term(Md, s1, s2));
+            ++nsel;
+        }
+    }
+    if (!p.SK) return;
+    red[threadIdx.x] = part;
+    cnt[threadIdx.x] = nsel;
+    __syncthreads();
+    for (int o = kScalarThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            red[threadIdx.x] = __dadd_rn(red[threadIdx.x], red[threadIdx.x + o]);
+            cnt[threadIdx.x] += cnt[threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double N = (double)cnt[0];
+        const float sk = eq14_sk(red[0], Md, N);
+        p.SK[cell] = sk;
+        if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, N));
+    }
+}
+
+// ------------------------------------------------------------------------------------- a7
+__global__ void sk_flag_kernel(const float* __restrict__ SK, uint8_t* __restrict__ mask, size_t cells,
+                               float sk_mean, float thr) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < cells) mask[i] = flag_decision(SK[i], sk_mean, thr);
+}
+
+// ------------------------------------------------------------------------------------- a8
+// Excision: every byte of every flagged cell becomes 0x88 (the encoded 0+0i).
+// grid = (cells, row chunks); a CTA whose cell is clean exits at once.
+constexpr int kExciseRows = 32;
+
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+sk_excise_kernel(uint8_t* __restrict__ data, const uint8_t* __restrict__ mask, uint32_t F, uint32_t E,
+                 uint32_t M) {
+    const uint32_t cell = blockIdx.x;
+    if (mask[cell] == 0) return;
+    const uint32_t b = cell / F, f = cell % F;
+    const uint32_t j0 = blockIdx.y * kExciseRows;
+    const uint32_t j1 = min(M, j0 + kExciseRows);
+    const size_t rstride = (size_t)F * E;
+    uint8_t* base = data + ((size_t)b * M * F + f) * E;
+    if (VEC) {
+        const uint32_t vec_per_row = E / 16;
+        const uint32_t total = (j1 - j0) * vec_per_row;
+        const uint4 z = make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
+        for (uint32_t i = threadIdx.x; i < total; i += blockDim.x) {
+            const uint32_t j = j0 + i / vec_per_row, c = i % vec_per_row;
+            reinterpret_cast<uint4*>(base + (size_t)j * rstride)[c] = z;
+        }
+    } else {
+        const uint32_t total = (j1 - j0) * E;
+        for (uint32_t i = threadIdx.x; i < total; i += blockDim.x) {
+            const uint32_t j = j0 + i / E, c = i % E;
+            base[(size_t)j * rstride + c] = 0x88;
+        }
+    }
+}
+
+}  // namespace sk

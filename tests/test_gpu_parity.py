@@ -1,0 +1,267 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded bytes.  Bar (BASELINE.json north_star): S1, S2 and mask bit-exact; SK within 1e-6
+relative, written as |gpu - ref| <= 1e-6 * max(1, |ref|).
+"""
+import numpy as np
+import pytest
+import torch
+
+import sk_synth
+
+pytestmark = pytest.mark.gpu
+
+SK_RTOL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def sk():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1808_10365_b200 as m
+    m.lib()
+    return m
+
+
+def u32np(t):
+    """uint32 CUDA tensor (or a slice of one) -> numpy uint32, via an int32 view."""
+    if t.dtype == torch.uint32:
+        t = t.view(torch.int32)
+    return t.contiguous().cpu().numpy().view(np.uint32)
+
+
+def assert_sk_close(gpu, ref):
+    gpu = np.asarray(gpu, np.float64)
+    ref = np.asarray(ref, np.float64)
+    assert np.array_equal(np.isnan(gpu), np.isnan(ref))
+    ok = ~np.isnan(ref)
+    err = np.abs(gpu[ok] - ref[ok])
+    tol = SK_RTOL * np.maximum(1.0, np.abs(ref[ok]))
+    assert (err <= tol).all(), f"max SK error {err.max():.3e}"
+
+
+def check_frame(sk, oracle, data_cpu, M, *, subset=None, first_n=None, n_sigma=3.0, sk_mean=1.0,
+                zero=False, data_gpu=None):
+    """Run fused (with sums) on the GPU and the oracle on the same bytes; compare everything."""
+    ref = oracle.frame(data_cpu.numpy(), M, subset=subset, first_n=first_n, n_sigma=n_sigma,
+                       sk_mean=sk_mean, zero_flagged=zero)
+    d = data_cpu.cuda() if data_gpu is None else data_gpu
+    out = sk.sk_frame(d, M, subset=subset, first_n=first_n, n_sigma=n_sigma, sk_mean=sk_mean,
+                      zero_flagged=zero, want_sums=True)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(u32np(out.S1), ref["S1"])
+    np.testing.assert_array_equal(u32np(out.S2), ref["S2"])
+    assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
+    np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])       # excised (or untouched) bytes
+    return out, ref
+
+
+SHAPES = [
+    # T, F, E, M — several tiles and ragged tails of every kind
+    (8, 1, 16, 2), (21, 2, 16, 7), (128, 3, 48, 64), (500, 1, 256, 250), (512, 2, 272, 256),
+    (768, 1, 2048, 256), (512, 3, 2064, 128), (2048, 1, 512, 1024), (2000, 2, 96, 1000),
+    (1024, 5, 32, 512), (66, 1, 4096, 33),
+]
+
+
+@pytest.mark.parametrize("T,F,E,M", SHAPES)
+def test_random_bytes_all_outputs(sk, oracle, T, F, E, M):
+    """Uniform random bytes: every nibble value incl. 0 (= -8, reading A3) occurs."""
+    data = sk_synth.random_bytes(T, F, E, seed=T * 31 + E)
+    data[: M, 0, : min(E, 16)] = 0x88                      # dead inputs in one cell (A4)
+    check_frame(sk, oracle, data, M, n_sigma=2.0, sk_mean=0.4)
+
+
+@pytest.mark.parametrize("T,F,E,M", [(512, 2, 272, 256), (768, 1, 2048, 256), (128, 3, 48, 64)])
+def test_receiver_selection(sk, oracle, T, F, E, M):
+    data = sk_synth.random_bytes(T, F, E, seed=7)
+    for first_n in (1, 15, 16, 17, E // 2 + 3, E):
+        check_frame(sk, oracle, data, M, first_n=first_n, sk_mean=0.5)
+    rng = np.random.default_rng(3)
+    for _ in range(3):
+        sub = rng.random(E) < 0.37
+        sub[rng.integers(E)] = True
+        check_frame(sk, oracle, data, M, subset=sub, sk_mean=0.5)
+    one = np.zeros(E, bool)
+    one[E - 1] = True
+    check_frame(sk, oracle, data, M, subset=one, sk_mean=0.5)
+
+
+@pytest.mark.parametrize("T,F,E,M", [(64, 2, 5, 8), (300, 1, 100, 100), (512, 3, 250, 256)])
+def test_scalar_fallback_shapes(sk, oracle, T, F, E, M):
+    """E % 16 != 0 takes the scalar kernel: same contract."""
+    data = sk_synth.random_bytes(T, F, E, seed=11)
+    check_frame(sk, oracle, data, M, sk_mean=0.5, zero=True)
+    check_frame(sk, oracle, data, M, first_n=max(1, E // 3), sk_mean=0.5)
+
+
+def test_misaligned_data_pointer(sk, oracle):
+    T, F, E, M = 256, 2, 64, 128
+    data = sk_synth.random_bytes(T, F, E, seed=12)
+    flat = torch.empty(T * F * E + 1, dtype=torch.uint8, device="cuda")
+    view = flat[1:].view(T, F, E)
+    view.copy_(data)
+    assert view.data_ptr() % 16 != 0
+    check_frame(sk, oracle, data, M, sk_mean=0.5, zero=True, data_gpu=view)
+
+
+def test_config0_toy(sk, oracle):
+    """BASELINE.json config 0: E=256, T=4096, M=256, CW in block 7, N=256, 3 sigma."""
+    cfg = sk_synth.config(0)
+    data = sk_synth.make_frame(cfg)
+    out, ref = check_frame(sk, oracle, data, cfg.M, n_sigma=3.0, sk_mean=1.0)
+    assert ref["mask"].all()          # literal centre 1.0: the 4-bit null mean (0.94) is > 3 sigma off
+    null = sk_synth.make_frame(cfg.with_(cw_block_inputs=None), frame=1)
+    null_mean = float(oracle.frame(null.numpy(), cfg.M)["SK"].mean())       # the paper's way
+    out, ref = check_frame(sk, oracle, data, cfg.M, n_sigma=3.0, sk_mean=null_mean)
+    assert ref["mask"][7, 0] == 1 and ref["mask"].sum() <= 2
+
+
+def test_config1_full_frame(sk, oracle):
+    """BASELINE.json config 1, full size (96 MiB, 192 cells), in the launch configuration bench.py
+    times (default arguments, no sums requested) plus a second run with sums."""
+    cfg = sk_synth.config(1)
+    data = sk_synth.make_frame(cfg, device="cuda")
+    out = sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
+    torch.cuda.synchronize()
+    host = data.cpu()
+    ref = oracle.frame(host.numpy(), cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
+    assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
+    np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    out2 = sk.sk_frame(data, cfg.M, want_sums=True)
+    np.testing.assert_array_equal(u32np(out2.S1), ref["S1"])
+    np.testing.assert_array_equal(u32np(out2.S2), ref["S2"])
+    assert torch.equal(out2.SK, out.SK)
+    # null distribution on 4-bit data: constant offset from 1, spread below first order
+    skv = ref["SK"].astype(np.float64).ravel()
+    assert 0.90 < skv.mean() < 0.93 and skv.std() < 1.2 * np.sqrt(4 / (cfg.M * cfg.E))
+
+
+def _check_sampled_cells(sk, oracle, data, out, M, cells, n_sigma, sk_mean, first_n=None):
+    T, F, E = data.shape
+    for (b, f) in cells:
+        cell = data[b * M:(b + 1) * M, f:f + 1, :].contiguous().cpu()
+        ref = oracle.frame(cell.numpy(), M, n_sigma=n_sigma, sk_mean=sk_mean, first_n=first_n)
+        assert_sk_close(out.SK[b, f].item(), ref["SK"][0, 0])
+        assert out.mask[b, f].item() == ref["mask"][0, 0]
+        if out.S1 is not None:
+            np.testing.assert_array_equal(u32np(out.S1.view(torch.int32)[b, f]), ref["S1"][0, 0])
+            np.testing.assert_array_equal(u32np(out.S2.view(torch.int32)[b, f]), ref["S2"][0, 0])
+
+
+def test_config2_rfi_mix_sampled(sk, oracle):
+    """Config 2 at full size (1 GiB): sampled cells against the oracle one by one, and the
+    injected interference is found."""
+    cfg = sk_synth.config(2)
+    data = sk_synth.make_frame(cfg, device="cuda")
+    null = sk_synth.make_frame(cfg.with_(T=4 * cfg.M, cw_freqs=(), burst_fraction=0.0, sine_freqs=()),
+                               device="cuda", frame=3)
+    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())
+    out = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, want_sums=True)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(2)
+    inj = sk_synth.rfi_cells(cfg).numpy()
+    cells = [(int(rng.integers(cfg.B)), int(rng.integers(cfg.F))) for _ in range(40)]
+    cells += [(int(b), 13) for b in rng.integers(cfg.B, size=4)] + [(0, 0), (cfg.B - 1, cfg.F - 1)]
+    _check_sampled_cells(sk, oracle, data, out, cfg.M, cells, 5.0, sk_mean)
+    mask = out.mask.cpu().numpy().astype(bool)
+    assert mask[inj].mean() > 0.99                  # CW, bursts and the 64-input sinusoid are all found
+    assert mask[~inj].mean() < 0.01
+    # excision of exactly the flagged cells, checked at full size with torch reductions only
+    before = data.clone()
+    out_z = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)
+    torch.cuda.synchronize()
+    assert torch.equal(out_z.mask, out.mask) and torch.equal(out_z.SK, out.SK)
+    cellview = data.view(cfg.B, cfg.M, cfg.F, cfg.E)
+    m = out.mask.bool()[:, None, :, None]
+    assert bool(((cellview == 0x88) | ~m).all())
+    assert bool(((cellview == before.view_as(cellview)) | m).all())
+    again = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)   # idempotent
+    assert torch.equal(again.mask, out.mask)
+    assert bool((again.SK[out.mask.bool()] == 0).all())
+
+
+def test_config3_sweep_sampled(sk, oracle):
+    """Config 3 (512 MiB): M x N sweep, sampled cells per point, and the closed-form trend."""
+    cfg = sk_synth.config(3)
+    data = sk_synth.make_frame(cfg, device="cuda")
+    rng = np.random.default_rng(3)
+    for M in (64, 128, 256, 512, 1024):
+        for N in (16, 64, 256, 1024, 2048):
+            out = sk.sk_frame(data, M, first_n=N, n_sigma=3.0, sk_mean=0.94)
+            B = cfg.T // M
+            cells = [(int(rng.integers(B)), int(rng.integers(cfg.F))) for _ in range(3)]
+            _check_sampled_cells(sk, oracle, data, out, M, cells, 3.0, 0.94, first_n=N)
+            skv = out.SK.double()
+            assert abs(skv.mean().item() - 0.941) < 0.01 + 4.0 / M         # 4-bit null mean (sigma 2.5)
+            ratio = skv.var().item() / (4.0 / (M * N))
+            assert 0.4 < ratio < 0.9                                       # below first order on 4-bit data
+
+
+def test_unfused_equals_fused(sk, oracle):
+    """sk_power_sums -> sk_combine -> sk_flag gives the fused call's bits (same summation order)."""
+    for (T, F, E, M) in [(512, 2, 272, 256), (768, 1, 2048, 256), (300, 1, 100, 100)]:
+        data = sk_synth.random_bytes(T, F, E, seed=5).cuda()
+        fused = sk.sk_frame(data, M, n_sigma=2.0, sk_mean=0.4, want_sums=True)
+        S1, S2 = sk.sk_power_sums(data, M)
+        SK = sk.sk_combine(S1, S2, M)
+        mask = sk.sk_flag(SK, M, E, 2.0, 0.4)
+        torch.cuda.synchronize()
+        assert torch.equal(S1.view(torch.int32), fused.S1.view(torch.int32))
+        assert torch.equal(S2.view(torch.int32), fused.S2.view(torch.int32))
+        assert torch.equal(SK.view(torch.int32), fused.SK.view(torch.int32))
+        assert torch.equal(mask, fused.mask)
+        ref = oracle.frame(data.cpu().numpy(), M, n_sigma=2.0, sk_mean=0.4)
+        assert_sk_close(SK.cpu().numpy(), ref["SK"])
+        sub = (np.arange(E) % 3 != 0)
+        SKs = sk.sk_combine(S1, S2, M, subset=sub)
+        fs = sk.sk_frame(data, M, subset=sub)
+        assert torch.equal(SKs.view(torch.int32), fs.SK.view(torch.int32))
+
+
+def test_deterministic_and_workspace_clean(sk):
+    data = sk_synth.random_bytes(1024, 2, 2048, seed=9).cuda()
+    ws = sk.workspace_for(1024, 2, 2048, 256, data.device, 12345)
+    a = sk.sk_frame(data, 256, workspace=ws)
+    torch.cuda.synchronize()
+    nparts = (1024 // 256) * 2 * (2048 // 256)
+    assert int(ws.view(torch.int32)[2 * nparts:].abs().sum().item()) == 0     # counters back to zero
+    for _ in range(5):
+        b = sk.sk_frame(data, 256, workspace=ws)
+        assert torch.equal(a.SK.view(torch.int32), b.SK.view(torch.int32))
+        assert torch.equal(a.mask, b.mask)
+
+
+def test_empty_subset_is_nan_and_flagged(sk):
+    data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
+    out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
+    assert bool(torch.isnan(out.SK).all()) and bool((out.mask == 1).all())
+
+
+def test_argument_errors(sk):
+    d = torch.zeros(64, 1, 32, dtype=torch.uint8, device="cuda")
+    for kw, code in [(dict(M=1), -3), (dict(M=48), -2), (dict(M=32, first_n=33), -4),
+                     (dict(M=32, first_n=0), -4), (dict(M=32, n_sigma=float("nan")), -5),
+                     (dict(M=32, workspace=torch.zeros(1, dtype=torch.int64, device="cuda")), -6)]:
+        with pytest.raises(sk.SKError) as ei:
+            sk.sk_frame(d, **kw)
+        assert f"({code})" in str(ei.value)
+    with pytest.raises(sk.SKError):
+        sk.sk_frame(torch.zeros(64, 1, 32, dtype=torch.uint8), 32)          # CPU tensor: no fallback
+
+
+def test_host_entry_point(sk, oracle):
+    cfg = sk_synth.config(0)
+    host = sk_synth.make_frame(cfg).pin_memory()
+    B, F = cfg.B, cfg.F
+    h_SK = torch.empty(B, F, dtype=torch.float32).pin_memory()
+    h_mask = torch.empty(B, F, dtype=torch.uint8).pin_memory()
+    d_data = torch.empty_like(host, device="cuda")
+    d_SK = torch.empty(B, F, dtype=torch.float32, device="cuda")
+    d_mask = torch.empty(B, F, dtype=torch.uint8, device="cuda")
+    ref = oracle.frame(host.numpy(), cfg.M, n_sigma=3.0, sk_mean=0.94, zero_flagged=True)
+    sk.sk_frame_host(host, cfg.M, h_SK, h_mask, d_data, d_SK, d_mask, n_sigma=3.0, sk_mean=0.94,
+                     zero_flagged=True)
+    assert_sk_close(h_SK.numpy(), ref["SK"])
+    np.testing.assert_array_equal(h_mask.numpy(), ref["mask"])
+    np.testing.assert_array_equal(host.numpy(), ref["data"])
