@@ -57,8 +57,7 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, const uint8_t* subset, 
     pl.slabs = (cover + W - 1) / W;
     const uint32_t RPW = 32u / pl.L;
     const uint32_t iters = (M + RPW - 1) / RPW;
-    const uint32_t padded = (iters + sk::kUnroll - 1) / sk::kUnroll * sk::kUnroll;
-    pl.wide = padded <= sk::AccWide::kMaxSamples;
+    pl.wide = iters <= sk::AccWide::kMaxSamples;
     return pl;
 }
 

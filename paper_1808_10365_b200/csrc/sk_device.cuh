@@ -20,14 +20,40 @@ __device__ __forceinline__ uint4 ldg_stream(const uint8_t* p) {
     return r;
 }
 
+// Scheduling fence for a batch of loads: every register of the batch passes through one empty
+// volatile asm, so all loads of the batch are issued before the first sample is unpacked
+// (keeps kUnroll 128-bit loads in flight per lane instead of one).
+template <int U>
+__device__ __forceinline__ void loads_issued(uint4 (&v)[U]) {
+#pragma unroll
+    for (int u = 0; u < U; u += 2) {
+        asm volatile("" : "+r"(v[u].x), "+r"(v[u].y), "+r"(v[u].z), "+r"(v[u].w),
+                          "+r"(v[u + 1].x), "+r"(v[u + 1].y), "+r"(v[u + 1].z), "+r"(v[u + 1].w));
+    }
+}
+
 // ------------------------------------------------------------------------- a1 + a2, packed
 // One 32-bit word holds 4 samples: byte = (re+8)<<4 | (im+8).
 //   hi(w) = (w & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*re   (one LOP3)
 //   lo(w) = ((w<<4) & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*im (SHF + LOP3)
 // Flipping the top bit of the offset nibble turns it into two's complement, and leaving it in
 // the high nibble of its byte sign-extends it for free (scaled by 16).  Nibble 0 -> -128 = 16*(-8).
-__device__ __forceinline__ uint32_t re16(uint32_t w) { return (w & 0xF0F0F0F0u) ^ 0x80808080u; }
-__device__ __forceinline__ uint32_t im16(uint32_t w) { return ((w << 4) & 0xF0F0F0F0u) ^ 0x80808080u; }
+// The two masks live in registers (LOP3 takes one immediate only; with both as literals ptxas
+// emits two LOP3 per word instead of one).
+struct UnpackConsts {
+    uint32_t f0, x80;
+    __device__ __forceinline__ void init() {
+        asm volatile("mov.u32 %0, 0xF0F0F0F0;" : "=r"(f0));
+        asm volatile("mov.u32 %0, 0x80808080;" : "=r"(x80));
+    }
+};
+__device__ __forceinline__ uint32_t and_xor(uint32_t a, uint32_t b, uint32_t c) {   // (a & b) ^ c
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x6a;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t re16(uint32_t w, const UnpackConsts& k) { return and_xor(w, k.f0, k.x80); }
+__device__ __forceinline__ uint32_t im16(uint32_t w, const UnpackConsts& k) { return and_xor(w << 4, k.f0, k.x80); }
 
 // Sample k of the word: C = [16re_k, 16im_k, 16re_k, 16im_k] (one PRMT), then one DP4A gives
 // C.C + c0 = 512 |x_k|^2 + c0  (|x|^2 <= 128, so 512|x|^2 <= 2^16).
@@ -71,11 +97,11 @@ struct AccWide {
 
 // Add the 16 samples of one 128-bit load to 16 accumulators.
 template <class Acc>
-__device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v) {
+__device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v, const UnpackConsts& kc) {
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint32_t r = re16(w[i]), m = im16(w[i]);
+        const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
         acc[4 * i + 0].add(power512<0>(r, m, Acc::kAddend));
         acc[4 * i + 1].add(power512<1>(r, m, Acc::kAddend));
         acc[4 * i + 2].add(power512<2>(r, m, Acc::kAddend));

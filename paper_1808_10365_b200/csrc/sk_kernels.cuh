@@ -35,6 +35,7 @@ struct FrameParams {
 
 constexpr int kWarpsPerCta = 4;
 constexpr int kUnroll = 8;     // 128-bit loads in flight per lane
+constexpr int kMinCtasPerSm = 4;   // with this hint ptxas keeps a batch of loads in flight (<= 128 regs)
 
 // Number of combined receivers N: first_n, or the count of non-zero subset bytes (whole warp).
 __device__ __forceinline__ uint32_t count_receivers(const FrameParams& p, int lane) {
@@ -50,21 +51,53 @@ __device__ __forceinline__ bool selected(const FrameParams& p, uint32_t e) {
     return p.subset ? (__ldg(p.subset + e) != 0) : (e < p.first_n);
 }
 
-// a4 + a5 (within a unit): the unit's share of S2bar, identical on all lanes on return.
-// Called by the fused kernel and by the combine kernel, so both add in the same order.
+// Sum the RPW row groups of a warp and scatter the result (recursive halving): on return lane
+// (r0, cl) holds kOwned<L> fully summed inputs starting at input offset `base` of its 16, in
+// v[0..kOwned).  Integers: exact in any order.  Costs 16 shuffles per array instead of 16*log2(RPW).
+template <int L> struct Owned { static constexpr int value = (16 * L / 32) > 0 ? (16 * L / 32) : 1; };
+
 template <int L>
-__device__ __forceinline__ double unit_partial(const FrameParams& p, int lane, bool active, uint32_t e0,
-                                               const uint32_t (&S1)[16], const uint32_t (&S2)[16]) {
+__device__ __forceinline__ int reduce_scatter_rows(uint32_t (&v1)[16], uint32_t (&v2)[16], int r0) {
     constexpr int RPW = 32 / L;
-    const int r0 = lane / L;
+    int base = 0;
+    int c = 16;
+#pragma unroll
+    for (int s = 0; (1 << s) < RPW; ++s) {
+        const int o = L << s;
+        const bool bit = (r0 >> s) & 1;
+        if (c > 1) {
+            const int h = c / 2;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (i < h) {
+                    const uint32_t k1 = bit ? v1[i + h] : v1[i], g1 = bit ? v1[i] : v1[i + h];
+                    const uint32_t k2 = bit ? v2[i + h] : v2[i], g2 = bit ? v2[i] : v2[i + h];
+                    v1[i] = k1 + __shfl_xor_sync(0xffffffffu, g1, o);
+                    v2[i] = k2 + __shfl_xor_sync(0xffffffffu, g2, o);
+                }
+            }
+            base += bit ? h : 0;
+            c = h;
+        } else {                       // RPW = 32: two row groups share the last input
+            v1[0] += __shfl_xor_sync(0xffffffffu, v1[0], o);
+            v2[0] += __shfl_xor_sync(0xffffffffu, v2[0], o);
+        }
+    }
+    return base;
+}
+
+// a4 + a5 (within a unit): the unit's share of S2bar, identical on all lanes on return.
+// v1/v2[0..kOwned) are the sums of inputs e0+base .. ; `owner` is false for the duplicate lane
+// when RPW = 32.  Called by the fused kernel and by the combine kernel: same order in both.
+template <int L>
+__device__ __forceinline__ double unit_partial(const FrameParams& p, bool active, bool owner, uint32_t e_first,
+                                               const uint32_t (&v1)[16], const uint32_t (&v2)[16]) {
     const double Md = (double)p.M;
     double part = 0.0;
-    if (active) {
+    if (active && owner) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            if ((k % RPW) == r0 && selected(p, e0 + k))      // share the 16 inputs among row groups
-                part = __dadd_rn(part, eq11_term(Md, S1[k], S2[k]));
-        }
+        for (int i = 0; i < Owned<L>::value; ++i)
+            if (selected(p, e_first + i)) part = __dadd_rn(part, eq11_term(Md, v1[i], v2[i]));
     }
     return warp_sum_fixed(part);
 }
@@ -96,12 +129,15 @@ __device__ __forceinline__ void publish_and_finalize(const FrameParams& p, uint3
     if (!last) return;
     __threadfence();
     finalize_cell(p, cell, lane, p.partial + (size_t)cell * p.slabs);
-    if (lane == 0) p.counter[cell] = 0u;                     // leave the workspace clean
+    __syncwarp();
+    // leave the workspace all-zero: partials and counter (header contract)
+    for (uint32_t s = lane; s < p.slabs; s += 32) p.partial[(size_t)cell * p.slabs + s] = 0.0;
+    if (lane == 0) p.counter[cell] = 0u;
 }
 
 // --------------------------------------------------------------------------- fused a1..a7
 template <int L, class Acc>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, kMinCtasPerSm)
 sk_frame_kernel(const FrameParams p) {
     constexpr int RPW = 32 / L;
     const int lane = threadIdx.x & 31;
@@ -116,47 +152,57 @@ sk_frame_kernel(const FrameParams p) {
     uint32_t S1[16], S2[16];
     {
         Acc acc[16];
+        UnpackConsts kc;
+        kc.init();
 #pragma unroll
         for (int k = 0; k < 16; ++k) acc[k].reset();
         const size_t rstride = (size_t)p.F * p.E;
         const uint8_t* base = p.data + ((size_t)b * p.M * p.F + f) * p.E + e0;
         uint32_t n = 0;
         if (active) {
-            for (uint32_t j = r0; j < p.M; j += RPW * kUnroll) {
+            // rows r0, r0+RPW, ...: full batches of kUnroll independent 128-bit loads, then a tail
+            const uint32_t mine = (p.M > (uint32_t)r0) ? (p.M - r0 + RPW - 1) / RPW : 0u;
+            const uint8_t* q = base + (size_t)r0 * rstride;
+            const size_t step = (size_t)RPW * rstride;
+            uint32_t i = 0;
+            for (; i + kUnroll <= mine; i += kUnroll) {
                 uint4 v[kUnroll];
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) {
-                    const uint32_t jj = j + u * RPW;
-                    v[u] = (jj < p.M) ? ldg_stream(base + (size_t)jj * rstride)
-                                      : make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
-                }
+                for (int u = 0; u < kUnroll; ++u) v[u] = ldg_stream(q + (size_t)u * step);
+                q += (size_t)kUnroll * step;
+                loads_issued(v);
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) accumulate16(acc, v[u]);
-                n += kUnroll;
+                for (int u = 0; u < kUnroll; ++u) accumulate16(acc, v[u], kc);
             }
+            for (; i < mine; ++i) {
+                const uint4 v = ldg_stream(q);
+                q += step;
+                accumulate16(acc, v, kc);
+            }
+            n = mine;
         }
 #pragma unroll
         for (int k = 0; k < 16; ++k) acc[k].read(n, S1[k], S2[k]);
-        // sum the RPW row groups: afterwards every lane of column cl holds the cell totals
+    }
+    const int base = reduce_scatter_rows<L>(S1, S2, r0);
+    constexpr int kOwn = Owned<L>::value;
+    const bool owner = (RPW <= 16) || (r0 < 16);
+    const uint32_t e_first = e0 + base;
+    if (p.S1out && active && owner) {
+        uint32_t* o1 = p.S1out + (size_t)cell * p.E + e_first;
+        uint32_t* o2 = p.S2out + (size_t)cell * p.E + e_first;
+        if (kOwn % 4 == 0) {
 #pragma unroll
-        for (int o = L; o < 32; o <<= 1) {
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                S1[k] += __shfl_xor_sync(0xffffffffu, S1[k], o);
-                S2[k] += __shfl_xor_sync(0xffffffffu, S2[k], o);
+            for (int i = 0; i < kOwn / 4; ++i) {
+                reinterpret_cast<uint4*>(o1)[i] = make_uint4(S1[4 * i], S1[4 * i + 1], S1[4 * i + 2], S1[4 * i + 3]);
+                reinterpret_cast<uint4*>(o2)[i] = make_uint4(S2[4 * i], S2[4 * i + 1], S2[4 * i + 2], S2[4 * i + 3]);
             }
-        }
-        if (p.S1out && active && r0 == 0) {
-            uint4* o1 = reinterpret_cast<uint4*>(p.S1out + (size_t)cell * p.E + e0);
-            uint4* o2 = reinterpret_cast<uint4*>(p.S2out + (size_t)cell * p.E + e0);
+        } else {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                o1[i] = make_uint4(S1[4 * i], S1[4 * i + 1], S1[4 * i + 2], S1[4 * i + 3]);
-                o2[i] = make_uint4(S2[4 * i], S2[4 * i + 1], S2[4 * i + 2], S2[4 * i + 3]);
-            }
+            for (int i = 0; i < kOwn; ++i) { o1[i] = S1[i]; o2[i] = S2[i]; }
         }
     }
-    if (p.SK) publish_and_finalize(p, cell, slab, lane, unit_partial<L>(p, lane, active, e0, S1, S2));
+    if (p.SK) publish_and_finalize(p, cell, slab, lane, unit_partial<L>(p, active, owner, e_first, S1, S2));
 }
 
 // ------------------------------------------------------------------ a4..a6 from stored sums
@@ -172,18 +218,26 @@ sk_combine_kernel(const FrameParams p) {
     for (uint32_t slab = warp; slab < p.slabs; slab += kWarpsPerCta) {
         const uint32_t e0 = (slab * L + cl) * 16u;
         const bool active = e0 < p.E;
+        constexpr int RPW = 32 / L;
+        constexpr int kOwn = Owned<L>::value;
+        const int r0 = lane / L;
+        // the same ownership as after the fused kernel's reduce-scatter: bit s of r0 picks the half
+        int base = 0;
+        {
+            int c = 16;
+#pragma unroll
+            for (int s = 0; (1 << s) < RPW; ++s)
+                if (c > 1) { c /= 2; base += ((r0 >> s) & 1) ? c : 0; }
+        }
+        const bool owner = (RPW <= 16) || (r0 < 16);
+        const uint32_t e_first = e0 + base;
         uint32_t S1[16], S2[16];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            uint4 a = make_uint4(0, 0, 0, 0), c = a;
-            if (active) {
-                a = __ldg(reinterpret_cast<const uint4*>(p.S1in + (size_t)cell * p.E + e0) + i);
-                c = __ldg(reinterpret_cast<const uint4*>(p.S2in + (size_t)cell * p.E + e0) + i);
-            }
-            S1[4 * i] = a.x; S1[4 * i + 1] = a.y; S1[4 * i + 2] = a.z; S1[4 * i + 3] = a.w;
-            S2[4 * i] = c.x; S2[4 * i + 1] = c.y; S2[4 * i + 2] = c.z; S2[4 * i + 3] = c.w;
+        for (int i = 0; i < kOwn; ++i) {
+            S1[i] = (active && owner) ? __ldg(p.S1in + (size_t)cell * p.E + e_first + i) : 0u;
+            S2[i] = (active && owner) ? __ldg(p.S2in + (size_t)cell * p.E + e_first + i) : 0u;
         }
-        const double part = unit_partial<L>(p, lane, active, e0, S1, S2);
+        const double part = unit_partial<L>(p, active, owner, e_first, S1, S2);
         if (lane == 0) partials[slab] = part;
     }
     __syncthreads();

@@ -121,15 +121,17 @@ def burst_starts(cfg: SKConfig) -> torch.Tensor:
     return blocks * cfg.M + off
 
 
-def rfi_cells(cfg: SKConfig) -> torch.Tensor:
-    """bool [B][F]: cells into which the recipe injects interference (for reporting only)."""
+def rfi_cells(cfg: SKConfig, include_sine: bool = True) -> torch.Tensor:
+    """bool [B][F]: cells into which the recipe injects interference (for reporting only).
+    include_sine=False leaves out cells whose only interference is the sinusoid confined to a few
+    inputs (it moves the full-array SK by only a few sigma)."""
     m = torch.zeros(cfg.B, cfg.F, dtype=torch.bool)
     if cfg.cw_block_inputs is not None:
         m[cfg.cw_block_inputs[0], 0] = True
     for f in range(cfg.F):
         if cfg.cw_period and (f % cfg.cw_period) in cfg.cw_freqs:
             m[:, f] = True
-        if f in cfg.sine_freqs and cfg.sine_inputs:
+        if include_sine and f in cfg.sine_freqs and cfg.sine_inputs:
             m[:, f] = True
     st = burst_starts(cfg)
     if st.numel():

@@ -165,8 +165,13 @@ def test_config2_rfi_mix_sampled(sk, oracle):
     cells += [(int(b), 13) for b in rng.integers(cfg.B, size=4)] + [(0, 0), (cfg.B - 1, cfg.F - 1)]
     _check_sampled_cells(sk, oracle, data, out, cfg.M, cells, 5.0, sk_mean)
     mask = out.mask.cpu().numpy().astype(bool)
-    assert mask[inj].mean() > 0.99                  # CW, bursts and the 64-input sinusoid are all found
+    strong = sk_synth.rfi_cells(cfg, include_sine=False).numpy()
+    assert mask[strong].mean() > 0.99               # CW and broadband bursts are all found
     assert mask[~inj].mean() < 0.01
+    # the sinusoid lives in 64 of 2048 inputs: in the full-array SK it is a few-sigma effect, but
+    # combining only the affected receivers (receiver subsets) finds it in every block
+    sub = sk.sk_frame(data, cfg.M, first_n=cfg.sine_inputs, n_sigma=5.0, sk_mean=sk_mean)
+    assert sub.mask[:, 13].float().mean().item() > 0.99
     # excision of exactly the flagged cells, checked at full size with torch reductions only
     before = data.clone()
     out_z = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)
@@ -224,8 +229,7 @@ def test_deterministic_and_workspace_clean(sk):
     ws = sk.workspace_for(1024, 2, 2048, 256, data.device, 12345)
     a = sk.sk_frame(data, 256, workspace=ws)
     torch.cuda.synchronize()
-    nparts = (1024 // 256) * 2 * (2048 // 256)
-    assert int(ws.view(torch.int32)[2 * nparts:].abs().sum().item()) == 0     # counters back to zero
+    assert int(ws.abs().sum().item()) == 0          # partials and counters are all zero again
     for _ in range(5):
         b = sk.sk_frame(data, 256, workspace=ws)
         assert torch.equal(a.SK.view(torch.int32), b.SK.view(torch.int32))
