@@ -6,6 +6,10 @@
 
 #include "../../include/sk_b200.h"
 #include "sk_kernels.cuh"
+#include "sk_tma.cuh"
+
+#include <cstdlib>
+#include <cstring>
 
 namespace {
 
@@ -75,13 +79,76 @@ void launch_vec_L(int L, const sk::FrameParams& p, cudaStream_t st) {
     ++g_launches;
 }
 
+// ---- TMA path ---------------------------------------------------------------------------
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled() {
+    // resolved through the runtime, so the library has no link-time dependency on libcuda.so
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        (void)cudaGetLastError();
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+
+int sm_count() {
+    static int n = [] {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            v = 148;
+        return v > 0 ? v : 148;
+    }();
+    return n;
+}
+
+// SK_B200_PATH=ldg|tma forces one vector kernel (for tests and A/B timing); default: TMA when it applies.
+bool tma_wanted(const sk::FrameParams& p, int L) {
+    const char* e = std::getenv("SK_B200_PATH");
+    if (e && std::strcmp(e, "ldg") == 0) return false;
+    return L == 16 && p.E >= 256 && encode_tiled() != nullptr;
+}
+
+template <class Acc>
+int launch_tma(const sk::FrameParams& p, cudaStream_t st) {
+    CUtensorMap tmap;
+    const cuuint64_t gdim[2] = {(cuuint64_t)p.F * p.E, (cuuint64_t)p.T};
+    const cuuint64_t gstride[1] = {(cuuint64_t)p.F * p.E};
+    const cuuint32_t box[2] = {(cuuint32_t)sk::kTmaSlab, (cuuint32_t)sk::kTmaRows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode_tiled()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(p.data), gdim,
+                                      gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(sk::sk_frame_tma_kernel<Acc>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sk::kTmaSmemBytes);
+        attr_set = true;
+    }
+    unsigned grid = (unsigned)(sm_count() * sk::kTmaCtasPerSm);
+    if (grid > p.nunits) grid = p.nunits;
+    sk::sk_frame_tma_kernel<Acc><<<grid, sk::kTmaWarps * 32, sk::kTmaSmemBytes, st>>>(tmap, p);
+    ++g_launches;
+    return SK_OK;
+}
+
 int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
     const uint32_t cells = p.B * p.F;
     if (pl.vec) {
         p.slabs = pl.slabs;
         p.nunits = cells * pl.slabs;
-        if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
-        else         launch_vec_L<sk::AccPlain>(pl.L, p, st);
+        if (tma_wanted(p, pl.L)) {
+            const int rc = pl.wide ? launch_tma<sk::AccWide>(p, st) : launch_tma<sk::AccPlain>(p, st);
+            if (rc != SK_OK) return rc;
+        } else if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
+        else                launch_vec_L<sk::AccPlain>(pl.L, p, st);
     } else {
         sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);
         ++g_launches;
