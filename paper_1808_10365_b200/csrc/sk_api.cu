@@ -20,12 +20,20 @@ inline int launch_status() {
     return e == cudaSuccess ? SK_OK : (int)e;
 }
 
-// Lanes per row for the vector path: a function of E only, so that sk_combine and sk_frame
-// split a cell into the same units and add the float64 terms in the same order.
-inline int lanes_per_row(uint32_t E) {
+int sm_count();
+
+// Lanes per row for the vector path (slab width = 16*L inputs): a function of the shape (E and
+// the number of cells B*F) and of the device only, so that sk_combine and sk_frame split a cell
+// into the same units and add the float64 terms in the same order.  Wide 256-byte slabs when that
+// still gives every SM kWarpsWanted warps to run; otherwise narrower slabs (more, smaller units).
+constexpr uint32_t kWarpsWanted = 16;
+
+inline int lanes_per_row(uint32_t E, uint32_t cells) {
     const uint32_t vecs = E / 16;            // 128-bit vectors per row
-    int L = 16;                              // 256-byte slabs for wide arrays
+    int L = 16;
     while (L > 1 && (uint32_t)L > vecs) L >>= 1;
+    const unsigned long long want = (unsigned long long)sm_count() * kWarpsWanted;
+    while (L > 4 && (unsigned long long)cells * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
     return L;
 }
 
@@ -50,11 +58,11 @@ struct Plan {
     bool wide;            // AccWide usable (samples per lane <= 511)
 };
 
-Plan make_plan(const void* data, uint32_t E, uint32_t M, const uint8_t* subset, uint32_t first_n,
-               bool need_all_inputs) {
+Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t cells, const uint8_t* subset,
+               uint32_t first_n, bool need_all_inputs) {
     Plan pl{};
     pl.vec = vector_ok(data, E);
-    pl.L = lanes_per_row(E);
+    pl.L = lanes_per_row(E, cells);
     const uint32_t W = 16u * pl.L;
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
@@ -108,33 +116,46 @@ int sm_count() {
     return n;
 }
 
-// SK_B200_PATH=ldg|tma forces one vector kernel (for tests and A/B timing); default: TMA when it applies.
-bool tma_wanted(const sk::FrameParams& p, int L) {
+// SK_B200_PATH=ldg|tma forces one vector kernel (for tests and A/B timing); default: TMA when it applies
+// (the stream kernel keeps its sums in AccWide fields: at most 511 samples per lane and unit).
+bool tma_wanted(const Plan& pl) {
     const char* e = std::getenv("SK_B200_PATH");
     if (e && std::strcmp(e, "ldg") == 0) return false;
-    return L == 16 && p.E >= 256 && encode_tiled() != nullptr;
+    return pl.wide && encode_tiled() != nullptr;
 }
 
-template <class Acc>
-int launch_tma(const sk::FrameParams& p, cudaStream_t st) {
+template <int L>
+int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(sk::sk_stream_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sk::kStreamSmemBytes);
+        cudaFuncSetAttribute(sk::sk_stream_kernel<L>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
+        attr_set = true;
+    }
+    sk::sk_stream_kernel<L><<<p.nunits, 32, sk::kStreamSmemBytes, st>>>(tmap, p);
+    return SK_OK;
+}
+
+int launch_stream(int L, const sk::FrameParams& p, cudaStream_t st) {
     CUtensorMap tmap;
+    const uint32_t W = 16u * L;
     const cuuint64_t gdim[2] = {(cuuint64_t)p.F * p.E, (cuuint64_t)p.T};
     const cuuint64_t gstride[1] = {(cuuint64_t)p.F * p.E};
-    const cuuint32_t box[2] = {(cuuint32_t)sk::kTmaSlab, (cuuint32_t)sk::kTmaRows};
+    const cuuint32_t box[2] = {(cuuint32_t)W, (cuuint32_t)(sk::kTileBytes / W)};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = encode_tiled()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(p.data), gdim,
                                       gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(sk::sk_frame_tma_kernel<Acc>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sk::kTmaSmemBytes);
-        attr_set = true;
+    switch (L) {
+        case 16: launch_stream_L<16>(tmap, p, st); break;
+        case 8:  launch_stream_L<8>(tmap, p, st); break;
+        case 4:  launch_stream_L<4>(tmap, p, st); break;
+        case 2:  launch_stream_L<2>(tmap, p, st); break;
+        default: launch_stream_L<1>(tmap, p, st); break;
     }
-    unsigned grid = (unsigned)(sm_count() * sk::kTmaCtasPerSm);
-    if (grid > p.nunits) grid = p.nunits;
-    sk::sk_frame_tma_kernel<Acc><<<grid, sk::kTmaWarps * 32, sk::kTmaSmemBytes, st>>>(tmap, p);
     ++g_launches;
     return SK_OK;
 }
@@ -144,8 +165,8 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
     if (pl.vec) {
         p.slabs = pl.slabs;
         p.nunits = cells * pl.slabs;
-        if (tma_wanted(p, pl.L)) {
-            const int rc = pl.wide ? launch_tma<sk::AccWide>(p, st) : launch_tma<sk::AccPlain>(p, st);
+        if (tma_wanted(pl)) {
+            const int rc = launch_stream(pl.L, p, st);
             if (rc != SK_OK) return rc;
         } else if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
         else                launch_vec_L<sk::AccPlain>(pl.L, p, st);
@@ -168,7 +189,7 @@ int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint3
                   uint32_t* S1, uint32_t* S2, void* stream) {
     if (!data || !S1 || !S2) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
-    Plan pl = make_plan(data, E, M, nullptr, E, true);
+    Plan pl = make_plan(data, E, M, (T / M) * F, nullptr, E, true);
     if ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
@@ -180,9 +201,7 @@ int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint3
 size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M) {
     if (check_shape(T, F, E, M)) return 0;
     const uint32_t cells = (T / M) * F;
-    const int L = lanes_per_row(E);
-    const uint32_t slabs = (E + 16u * L - 1) / (16u * L);
-    return workspace_bytes(cells, slabs);
+    return workspace_bytes(cells, (E + 15u) / 16u);     // room for the narrowest slabs any plan uses
 }
 
 static int frame_impl(const uint8_t* data, uint32_t T,
@@ -194,7 +213,7 @@ static int frame_impl(const uint8_t* data, uint32_t T,
     if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
     if (mask && (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0)) return SK_ERR_PARAM;
     if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
-    Plan pl = make_plan(data, E, M, subset, first_n, S1o != nullptr);
+    Plan pl = make_plan(data, E, M, (T / M) * F, subset, first_n, S1o != nullptr);
     if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
@@ -208,9 +227,8 @@ static int frame_impl(const uint8_t* data, uint32_t T,
             return SK_ERR_WORKSPACE;
         p.partial = static_cast<double*>(workspace);
         // counters sit after the largest possible partial array, so their place does not depend
-        // on first_n and a workspace stays clean across calls with different receiver subsets
-        const int L = pl.L;
-        const uint32_t slabs_max = (E + 16u * L - 1) / (16u * L);
+        // on first_n or on the slab width and a workspace stays clean across calls
+        const uint32_t slabs_max = (E + 15u) / 16u;
         if (workspace_bytes_given < workspace_bytes(cells, slabs_max)) return SK_ERR_WORKSPACE;
         p.counter = reinterpret_cast<uint32_t*>(static_cast<double*>(workspace) + (size_t)cells * slabs_max);
     }
@@ -232,7 +250,7 @@ int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, u
     const bool vec = E % 16 == 0 &&
                      ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) == 0;
     if (vec) {
-        const int L = lanes_per_row(E);
+        const int L = lanes_per_row(E, cells);
         p.slabs = (E + 16u * L - 1) / (16u * L);
         p.nunits = cells * p.slabs;
         const size_t smem = (size_t)p.slabs * sizeof(double);

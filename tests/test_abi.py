@@ -58,10 +58,11 @@ def test_argument_errors_need_no_device(sk):
 
 
 def test_workspace_bytes(sk):
-    # cells * slabs doubles + cells counters; slabs = ceil(E / 256) for E >= 256
-    assert sk.sk_frame_workspace_bytes(49152, 1, 2048, 256) == 192 * 8 * 8 + 192 * 4
-    assert sk.sk_frame_workspace_bytes(4096, 1, 256, 256) == 16 * 1 * 8 + 16 * 4
-    assert sk.sk_frame_workspace_bytes(64, 2, 48, 32) == 4 * 2 * 8 + 4 * 4      # L = 2: 32-byte slabs
+    # cells * ceil(E/16) doubles (room for the narrowest slabs any plan uses) + cells counters:
+    # a function of the shape only, never of the device
+    assert sk.sk_frame_workspace_bytes(49152, 1, 2048, 256) == 192 * 128 * 8 + 192 * 4
+    assert sk.sk_frame_workspace_bytes(4096, 1, 256, 256) == 16 * 16 * 8 + 16 * 4
+    assert sk.sk_frame_workspace_bytes(64, 2, 48, 32) == 4 * 3 * 8 + 4 * 4
     assert sk.sk_frame_workspace_bytes(10, 1, 16, 4) == 0                        # T % M != 0
 
 
