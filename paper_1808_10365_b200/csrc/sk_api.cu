@@ -28,12 +28,15 @@ int sm_count();
 // still gives every SM kWarpsWanted warps to run; otherwise narrower slabs (more, smaller units).
 constexpr uint32_t kWarpsWanted = 16;
 
-inline int lanes_per_row(uint32_t E, uint32_t cells) {
+inline int lanes_per_row(uint32_t E, uint32_t cells, uint32_t M) {
     const uint32_t vecs = E / 16;            // 128-bit vectors per row
     int L = 16;
     while (L > 1 && (uint32_t)L > vecs) L >>= 1;
     const unsigned long long want = (unsigned long long)sm_count() * kWarpsWanted;
     while (L > 4 && (unsigned long long)cells * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
+    // long blocks: narrower slabs put more rows under one warp-wide read, so that a lane still
+    // adds at most AccChain::kMaxSamples samples per unit (the stream kernel's exactness limit)
+    while (L > 1 && (M + 32u / L - 1) / (32u / L) > sk::AccChain::kMaxSamples) L >>= 1;
     return L;
 }
 
@@ -56,13 +59,14 @@ struct Plan {
     int L;
     uint32_t slabs;       // launched slabs per cell
     bool wide;            // AccWide usable (samples per lane <= 511)
+    bool stream;          // stream kernel usable (samples per lane <= 128)
 };
 
 Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t cells, const uint8_t* subset,
                uint32_t first_n, bool need_all_inputs) {
     Plan pl{};
     pl.vec = vector_ok(data, E);
-    pl.L = lanes_per_row(E, cells);
+    pl.L = lanes_per_row(E, cells, M);
     const uint32_t W = 16u * pl.L;
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
@@ -70,6 +74,7 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t cells, const u
     const uint32_t RPW = 32u / pl.L;
     const uint32_t iters = (M + RPW - 1) / RPW;
     pl.wide = iters <= sk::AccWide::kMaxSamples;
+    pl.stream = iters <= sk::AccChain::kMaxSamples;
     return pl;
 }
 
@@ -121,7 +126,7 @@ int sm_count() {
 bool tma_wanted(const Plan& pl) {
     const char* e = std::getenv("SK_B200_PATH");
     if (e && std::strcmp(e, "ldg") == 0) return false;
-    return pl.wide && encode_tiled() != nullptr;
+    return pl.stream && encode_tiled() != nullptr;
 }
 
 template <int L>
@@ -250,7 +255,7 @@ int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, u
     const bool vec = E % 16 == 0 &&
                      ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) == 0;
     if (vec) {
-        const int L = lanes_per_row(E, cells);
+        const int L = lanes_per_row(E, cells, M);
         p.slabs = (E + 16u * L - 1) / (16u * L);
         p.nunits = cells * p.slabs;
         const size_t smem = (size_t)p.slabs * sizeof(double);

@@ -88,12 +88,46 @@ struct AccWide {
     static constexpr uint32_t kMaxSamples = 511;
     __device__ __forceinline__ void reset() { a = 0ull; }
     __device__ __forceinline__ void add(uint32_t q) { a += (unsigned long long)q * q; }
+    __device__ __forceinline__ void add_c(uint32_t c) { add((uint32_t)__dp4a((int)c, (int)c, (int)kAddend)); }
     __device__ __forceinline__ void read(uint32_t n, uint32_t& S1, uint32_t& S2) const {
         const unsigned long long v = a - ((unsigned long long)(n & 3u) << 62);
         S1 = (uint32_t)(v >> 41);
         S2 = (uint32_t)((v & ((1ull << 41) - 1ull)) >> 18);
     }
 };
+
+// AccChain: S1 on the IDP addend chain, S2 on the FP32 pipes (which the integer path leaves idle).
+//   r starts as the bit pattern of the float 2^23 and every IDP adds 512 p to it:
+//   r_k = IDP(C, C, r_{k-1}).  While 512 sum(p) <= 2^23 the float view of r is exactly
+//   2^23 + 512 sum(p), so d = float(r_k) - float(r_{k-1}) = 512 p_k exactly (one FADD) and
+//   s2 = fma(d, d, s2) = 2^18 sum(p^2) exactly (sum p^2 < 2^24).  S1 = (r - 2^23 pattern) >> 9.
+//   Limit: sum(p) <= 16384, i.e. n <= 128 samples per lane and unit (p <= 128).
+//   Why: IMAD.WIDE costs 4 cycles of the half-rate fmaheavy pipe, the bottleneck of an all-AccWide
+//   kernel (ncu: sm__pipe_fmaheavy_cycles_active 78 %); FADD/FFMA also run on fmalite.
+struct AccChain {
+    uint32_t r;
+    float s2;
+    static constexpr uint32_t kMagic = 0x4B000000u;
+    static constexpr uint32_t kMaxSamples = 128;
+    __device__ __forceinline__ void reset() { r = kMagic; s2 = 0.0f; }
+    __device__ __forceinline__ void add_c(uint32_t c) {
+        const uint32_t r2 = (uint32_t)__dp4a((int)c, (int)c, (int)r);
+        const float d = __fsub_rn(__uint_as_float(r2), __uint_as_float(r));
+        s2 = __fmaf_rn(d, d, s2);
+        r = r2;
+    }
+    __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const {
+        S1 = (r - kMagic) >> 9;
+        S2 = __float2uint_rn(s2 * (1.0f / 262144.0f));
+    }
+};
+
+// [16re_k, 16im_k, 16re_k, 16im_k] of sample K of a word (one PRMT).
+template <int K>
+__device__ __forceinline__ uint32_t pick(uint32_t r16, uint32_t i16) {
+    constexpr uint32_t sel = (uint32_t)K | ((4u + K) << 4) | ((uint32_t)K << 8) | ((4u + K) << 12);
+    return __byte_perm(r16, i16, sel);
+}
 
 // Add the 16 samples of one 128-bit load to 16 accumulators.
 template <class Acc>
@@ -106,6 +140,21 @@ __device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v, con
         acc[4 * i + 1].add(power512<1>(r, m, Acc::kAddend));
         acc[4 * i + 2].add(power512<2>(r, m, Acc::kAddend));
         acc[4 * i + 3].add(power512<3>(r, m, Acc::kAddend));
+    }
+}
+
+// The same with the accumulators split over the pipes: inputs 4i, 4i+1 of every word use the
+// accumulators A (8 of them), inputs 4i+2, 4i+3 the accumulators B.
+template <class AccA, class AccB>
+__device__ __forceinline__ void accumulate16_split(AccA (&a)[8], AccB (&b)[8], const uint4& v, const UnpackConsts& kc) {
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
+        a[2 * i + 0].add_c(pick<0>(r, m));
+        a[2 * i + 1].add_c(pick<1>(r, m));
+        b[2 * i + 0].add_c(pick<2>(r, m));
+        b[2 * i + 1].add_c(pick<3>(r, m));
     }
 }
 

@@ -92,9 +92,10 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
 
     UnpackConsts kc;
     kc.init();
-    AccWide acc[16];
+    AccWide accA[8];
+    AccChain accB[8];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) acc[k].reset();
+    for (int k = 0; k < 8; ++k) { accA[k].reset(); accB[k].reset(); }
     uint32_t n = 0, slot = 0, parity = 0;
     for (uint32_t t = 0; t < tiles; ++t) {
         const uint32_t bar = bars + 8 * slot;
@@ -103,11 +104,11 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
         const uint32_t rows = min((uint32_t)R, p.M - t * R);
         if (rows == (uint32_t)R) {
 #pragma unroll
-            for (int i = 0; i < NLD; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+            for (int i = 0; i < NLD; ++i) accumulate16_split(accA, accB, lds128(src + i * RPW * W), kc);
             n += NLD;
         } else {
             for (uint32_t r = r0; r < rows; r += RPW) {
-                accumulate16(acc, lds128(src + (r - r0) * W), kc);
+                accumulate16_split(accA, accB, lds128(src + (r - r0) * W), kc);
                 ++n;
             }
         }
@@ -121,10 +122,15 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
 
     uint32_t S1[16], S2[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        acc[k].read(n, S1[k], S2[k]);
-        if (!active) { S1[k] = 0; S2[k] = 0; }
+    for (int i = 0; i < 4; ++i) {
+        accA[2 * i + 0].read(n, S1[4 * i + 0], S2[4 * i + 0]);
+        accA[2 * i + 1].read(n, S1[4 * i + 1], S2[4 * i + 1]);
+        accB[2 * i + 0].read(n, S1[4 * i + 2], S2[4 * i + 2]);
+        accB[2 * i + 1].read(n, S1[4 * i + 3], S2[4 * i + 3]);
     }
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+        if (!active) { S1[k] = 0; S2[k] = 0; }
     const int base = reduce_scatter_rows<L>(S1, S2, r0);
     constexpr int kOwn = Owned<L>::value;
     const bool owner = (RPW <= 16) || (r0 < 16);
