@@ -60,11 +60,14 @@ struct Plan {
     uint32_t slabs;       // launched slabs per cell
     bool wide;            // AccWide usable (samples per lane <= 511)
     bool stream;          // stream kernel usable (samples per lane <= 128)
+    bool grid_ok;         // F and B fit the y and z grid dimensions
 };
 
-Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t cells, const uint8_t* subset,
+Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F, const uint8_t* subset,
                uint32_t first_n, bool need_all_inputs) {
     Plan pl{};
+    const uint32_t cells = B * F;
+    pl.grid_ok = B <= 65535u && F <= 65535u;
     pl.vec = vector_ok(data, E);
     pl.L = lanes_per_row(E, cells, M);
     const uint32_t W = 16u * pl.L;
@@ -126,7 +129,7 @@ int sm_count() {
 bool tma_wanted(const Plan& pl) {
     const char* e = std::getenv("SK_B200_PATH");
     if (e && std::strcmp(e, "ldg") == 0) return false;
-    return pl.stream && encode_tiled() != nullptr;
+    return pl.stream && pl.grid_ok && encode_tiled() != nullptr;
 }
 
 template <int L>
@@ -139,7 +142,7 @@ int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, cudaStrea
                              cudaSharedmemCarveoutMaxShared);
         attr_set = true;
     }
-    sk::sk_stream_kernel<L><<<p.nunits, 32, sk::kStreamSmemBytes, st>>>(tmap, p);
+    sk::sk_stream_kernel<L><<<dim3(p.slabs, p.F, p.B), 32, sk::kStreamSmemBytes, st>>>(tmap, p);
     return SK_OK;
 }
 
@@ -194,7 +197,7 @@ int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint3
                   uint32_t* S1, uint32_t* S2, void* stream) {
     if (!data || !S1 || !S2) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
-    Plan pl = make_plan(data, E, M, (T / M) * F, nullptr, E, true);
+    Plan pl = make_plan(data, E, M, T / M, F, nullptr, E, true);
     if ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
@@ -218,7 +221,7 @@ static int frame_impl(const uint8_t* data, uint32_t T,
     if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
     if (mask && (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0)) return SK_ERR_PARAM;
     if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
-    Plan pl = make_plan(data, E, M, (T / M) * F, subset, first_n, S1o != nullptr);
+    Plan pl = make_plan(data, E, M, T / M, F, subset, first_n, S1o != nullptr);
     if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;

@@ -143,20 +143,47 @@ __device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v, con
     }
 }
 
-// The same with the accumulators split over the pipes: inputs 4i, 4i+1 of every word use the
-// accumulators A (8 of them), inputs 4i+2, 4i+3 the accumulators B.
-template <class AccA, class AccB>
-__device__ __forceinline__ void accumulate16_split(AccA (&a)[8], AccB (&b)[8], const uint4& v, const UnpackConsts& kc) {
-    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+// The same with the accumulators split over the pipes: of the 4 inputs of every 32-bit word the
+// first NW use the AccWide accumulators a[], the other 4 - NW the AccChain accumulators b[].
+#ifndef SK_NWIDE
+#define SK_NWIDE 0
+#endif
+constexpr int kNWide = SK_NWIDE;                   // per word; measured on B200: 0 (all AccChain) is fastest
+
+struct AccSplit {
+    AccWide a[4 * kNWide > 0 ? 4 * kNWide : 1];
+    AccChain b[4 * (4 - kNWide) > 0 ? 4 * (4 - kNWide) : 1];
+    __device__ __forceinline__ void reset() {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
-        a[2 * i + 0].add_c(pick<0>(r, m));
-        a[2 * i + 1].add_c(pick<1>(r, m));
-        b[2 * i + 0].add_c(pick<2>(r, m));
-        b[2 * i + 1].add_c(pick<3>(r, m));
+        for (int k = 0; k < 4 * kNWide; ++k) a[k].reset();
+#pragma unroll
+        for (int k = 0; k < 4 * (4 - kNWide); ++k) b[k].reset();
     }
-}
+    template <int I, int K>
+    __device__ __forceinline__ void add_c(uint32_t c) {
+        if (K < kNWide) a[kNWide * I + K].add_c(c);
+        else            b[(4 - kNWide) * I + (K - kNWide)].add_c(c);
+    }
+    template <int I>
+    __device__ __forceinline__ void add_word(uint32_t w, const UnpackConsts& kc) {
+        const uint32_t r = re16(w, kc), m = im16(w, kc);
+        add_c<I, 0>(pick<0>(r, m));
+        add_c<I, 1>(pick<1>(r, m));
+        add_c<I, 2>(pick<2>(r, m));
+        add_c<I, 3>(pick<3>(r, m));
+    }
+    __device__ __forceinline__ void add16(const uint4& v, const UnpackConsts& kc) {
+        add_word<0>(v.x, kc);
+        add_word<1>(v.y, kc);
+        add_word<2>(v.z, kc);
+        add_word<3>(v.w, kc);
+    }
+    // sums of input 4*i + k of the lane's 16
+    __device__ __forceinline__ void read(int i, int k, uint32_t n, uint32_t& S1, uint32_t& S2) const {
+        if (k < kNWide) a[kNWide * i + k].read(n, S1, S2);
+        else            b[(4 - kNWide) * i + (k - kNWide)].read(n, S1, S2);
+    }
+};
 
 // Scalar a1-a2 for the fallback kernel.
 __device__ __forceinline__ uint32_t power_scalar(uint8_t byte) {
@@ -165,12 +192,35 @@ __device__ __forceinline__ uint32_t power_scalar(uint8_t byte) {
 }
 
 // ------------------------------------------------------------------------------------- a4
-// term = M^2 S2 / S1^2 in float64, every operation individually rounded (no FMA contraction);
-// a receiver with S1 == 0 contributes M (header: "A receiver whose S1 is 0 ...").
-__device__ __forceinline__ double eq11_term(double M, uint32_t S1, uint32_t S2) {
-    if (S1 == 0u) return M;
-    const double s1 = (double)S1, s2 = (double)S2;
-    return __ddiv_rn(__dmul_rn(__dmul_rn(M, M), s2), __dmul_rn(s1, s1));
+// uint32 -> float64 without the conversion unit: the integer is the low word of 2^52 + u.
+__device__ __forceinline__ double u32_to_f64(uint32_t u) {
+    return __dsub_rn(__hiloint2double(0x43300000, (int)u), 4503599627370496.0);
+}
+
+// n / y for 1 <= y < 2^53, 0 <= n < 2^60: hardware reciprocal seed, two Newton steps, one
+// correction of the quotient.  Branch-free; the result is within one ulp of n / y (normally the
+// correctly rounded quotient).  Every kernel divides through this one function, so all paths
+// agree bit for bit; against the oracle's IEEE division the difference is <= 2.2e-16 relative
+// per term, nine orders of magnitude inside the 1e-6 tolerance on SK.
+__device__ __forceinline__ double div_f64(double n, double y) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+    double e = __fma_rn(-y, r, 1.0);
+    r = __fma_rn(r, e, r);
+    e = __fma_rn(-y, r, 1.0);
+    r = __fma_rn(r, e, r);
+    e = __fma_rn(-y, r, 1.0);
+    r = __fma_rn(r, e, r);
+    const double q = __dmul_rn(n, r);
+    return __fma_rn(__fma_rn(-y, q, n), r, q);
+}
+
+// term = M^2 S2 / S1^2 in float64 (MM = M*M, exact); numerator and denominator are exact
+// integers below 2^53.  A receiver with S1 == 0 contributes M (header: "A receiver whose S1 is 0").
+__device__ __forceinline__ double eq11_term(double M, double MM, uint32_t S1, uint32_t S2) {
+    const double s1 = u32_to_f64(S1), s2 = u32_to_f64(S2);
+    const double t = div_f64(__dmul_rn(MM, s2), __dmul_rn(s1, s1));
+    return S1 == 0u ? M : t;
 }
 
 // a6: SK~ = (M+1)/(M-1) * (S2bar/(M N) - 1)  (Eq. 14, second line), then float32.

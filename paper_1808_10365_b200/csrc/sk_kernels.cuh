@@ -92,12 +92,14 @@ __device__ __forceinline__ int reduce_scatter_rows(uint32_t (&v1)[16], uint32_t 
 template <int L>
 __device__ __forceinline__ double unit_partial(const FrameParams& p, bool active, bool owner, uint32_t e_first,
                                                const uint32_t (&v1)[16], const uint32_t (&v2)[16]) {
-    const double Md = (double)p.M;
+    const double Md = (double)p.M, MM = __dmul_rn(Md, Md);
     double part = 0.0;
     if (active && owner) {
 #pragma unroll
-        for (int i = 0; i < Owned<L>::value; ++i)
-            if (selected(p, e_first + i)) part = __dadd_rn(part, eq11_term(Md, v1[i], v2[i]));
+        for (int i = 0; i < Owned<L>::value; ++i) {
+            const double t = eq11_term(Md, MM, v1[i], v2[i]);
+            part = __dadd_rn(part, selected(p, e_first + i) ? t : 0.0);
+        }
     }
     return warp_sum_fixed(part);
 }
@@ -276,7 +278,7 @@ __global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const Fr
             }
         }
         if (p.SK && selected(p, e)) {
-            part = __dadd_rn(part, eq11_term(Md, s1, s2));
+            part = __dadd_rn(part, eq11_term(Md, __dmul_rn(Md, Md), s1, s2));
             ++nsel;
         }
     }

@@ -16,9 +16,18 @@
 
 namespace sk {
 
-constexpr int kTileBytes = 4096;                   // bytes per TMA tile (R rows x W inputs)
-constexpr int kStages = 2;                         // tiles in flight per warp
-constexpr int kStreamMinCtas = 24;                 // resident warps per SM the register budget allows
+#ifndef SK_TILE_BYTES
+#define SK_TILE_BYTES 4096
+#endif
+#ifndef SK_STAGES
+#define SK_STAGES 2
+#endif
+#ifndef SK_MINCTAS
+#define SK_MINCTAS 24
+#endif
+constexpr int kTileBytes = SK_TILE_BYTES;          // bytes per TMA tile (R rows x W inputs)
+constexpr int kStages = SK_STAGES;                 // tiles in flight per warp
+constexpr int kStreamMinCtas = SK_MINCTAS;         // resident warps per SM the register budget allows
 constexpr size_t kStreamSmemBytes = (size_t)kStages * kTileBytes + kStages * 8;
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -64,10 +73,11 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
     const uint32_t ring = smem_addr(smem);
     const uint32_t bars = ring + kStages * kTileBytes;
 
-    const uint32_t unit = blockIdx.x;
-    const uint32_t slab = unit % p.slabs, cell = unit / p.slabs;
-    const uint32_t b = cell / p.F, f = cell % p.F;
+    // grid = (slabs, F, B): no integer division on the way to the first load
+    const uint32_t slab = blockIdx.x, f = blockIdx.y, b = blockIdx.z;
+    const uint32_t cell = b * p.F + f;
     const uint32_t x0 = f * p.E + slab * W, y0 = b * p.M;
+    const uint32_t full = p.M / R;                 // tiles with all R rows inside the block
     const uint32_t tiles = (p.M + R - 1) / R;
 
     if (lane == 0) {
@@ -92,45 +102,50 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
 
     UnpackConsts kc;
     kc.init();
-    AccWide accA[8];
-    AccChain accB[8];
+    AccSplit acc;
+    acc.reset();
+    uint32_t n = 0, t = 0, parity = 0;
+    uint32_t ynext = y0 + kStages * R;             // first row of the tile the next refill fetches
+    // rounds of kStages full tiles: slot numbers are compile-time constants
+    while (t + kStages <= full) {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) { accA[k].reset(); accB[k].reset(); }
-    uint32_t n = 0, slot = 0, parity = 0;
-    for (uint32_t t = 0; t < tiles; ++t) {
-        const uint32_t bar = bars + 8 * slot;
-        const uint32_t src = ring + slot * kTileBytes + lane_off;
-        mbar_wait(bar, parity);
-        const uint32_t rows = min((uint32_t)R, p.M - t * R);
-        if (rows == (uint32_t)R) {
+        for (int s = 0; s < kStages; ++s) {
+            const uint32_t bar = bars + 8 * s;
+            const uint32_t src = ring + s * kTileBytes + lane_off;
+            mbar_wait(bar, parity);
 #pragma unroll
-            for (int i = 0; i < NLD; ++i) accumulate16_split(accA, accB, lds128(src + i * RPW * W), kc);
-            n += NLD;
-        } else {
-            for (uint32_t r = r0; r < rows; r += RPW) {
-                accumulate16_split(accA, accB, lds128(src + (r - r0) * W), kc);
-                ++n;
+            for (int i = 0; i < NLD; ++i) acc.add16(lds128(src + i * RPW * W), kc);
+            __syncwarp();                          // every lane has consumed this slot: refill it
+            if (lane == 0 && t + s + kStages < tiles) {
+                mbar_expect_tx(bar, kTileBytes);
+                tma_load_tile(ring + s * kTileBytes, &tmap, x0, ynext + s * R, bar);
             }
         }
-        __syncwarp();                              // every lane has consumed this slot: refill it
-        if (lane == 0 && t + kStages < tiles) {
-            mbar_expect_tx(bar, kTileBytes);
-            tma_load_tile(ring + slot * kTileBytes, &tmap, x0, y0 + (t + kStages) * R, bar);
+        t += kStages;
+        ynext += kStages * R;
+        parity ^= 1;
+        n += kStages * NLD;
+    }
+    // what is left (fewer than kStages full tiles, then a ragged one) is already on its way
+    for (uint32_t s = 0; t < tiles; ++t, ++s) {
+        const uint32_t src = ring + s * kTileBytes + lane_off;
+        mbar_wait(bars + 8 * s, parity);
+        const uint32_t rows = min((uint32_t)R, p.M - t * R);
+        for (uint32_t r = r0; r < rows; r += RPW) {
+            acc.add16(lds128(src + (r - r0) * W), kc);
+            ++n;
         }
-        if (++slot == kStages) { slot = 0; parity ^= 1; }
     }
 
     uint32_t S1[16], S2[16];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        accA[2 * i + 0].read(n, S1[4 * i + 0], S2[4 * i + 0]);
-        accA[2 * i + 1].read(n, S1[4 * i + 1], S2[4 * i + 1]);
-        accB[2 * i + 0].read(n, S1[4 * i + 2], S2[4 * i + 2]);
-        accB[2 * i + 1].read(n, S1[4 * i + 3], S2[4 * i + 3]);
-    }
 #pragma unroll
-    for (int k = 0; k < 16; ++k)
-        if (!active) { S1[k] = 0; S2[k] = 0; }
+        for (int k = 0; k < 4; ++k) {
+            acc.read(i, k, n, S1[4 * i + k], S2[4 * i + k]);
+            if (!active) { S1[4 * i + k] = 0; S2[4 * i + k] = 0; }
+        }
+    }
     const int base = reduce_scatter_rows<L>(S1, S2, r0);
     constexpr int kOwn = Owned<L>::value;
     const bool owner = (RPW <= 16) || (r0 < 16);
