@@ -73,22 +73,35 @@ int sk_flag(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, flo
  * clearing.  Do not share one workspace between calls that may run concurrently. */
 size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M);
 
+/* Bits of sk_frame's `flags`. */
+#define SK_FRAME_ZERO_FLAGGED  1  /* a8: excise flagged cells in place */
+#define SK_FRAME_INPUTS_READY  2  /* see below */
+
 /* a1-a8 in one pass over HBM.  Writes SK and mask [T/M][F]; S1_opt / S2_opt [T/M][F][E] are
- * written when non-NULL.  If zero_flagged != 0, every byte (all E inputs, all M rows) of each
- * flagged cell is overwritten in place with 0x88 after the mask is known (the mask and SK are
- * those of the data before excision); otherwise `data` is only read. */
+ * written when non-NULL.  With SK_FRAME_ZERO_FLAGGED every byte (all E inputs, all M rows) of
+ * each flagged cell is overwritten in place with 0x88 after the mask is known (the mask and SK
+ * are those of the data before excision); otherwise `data` is only read.
+ * SK_FRAME_INPUTS_READY is a promise by the caller that `data` and `subset` are not written by
+ * the work enqueued on `stream` immediately before this call (e.g. the frame was uploaded and
+ * synchronised earlier, or lives in a buffer other than the one the previous call excised).
+ * The kernel is launched with programmatic stream serialization; with the promise it reads
+ * `data` while the previous kernel on the stream is still draining and waits for it only before
+ * its first write (outputs and workspace), so back-to-back frames overlap tail and ramp-up.
+ * Without the flag the kernel waits for the previous work before its first read.  Results are
+ * identical either way. */
 int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
              const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
-             int zero_flagged, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
+             int flags, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
              void* workspace, size_t workspace_bytes, void* stream);
 
 /* End-to-end form with HOST buffers (pinned memory recommended): copies h_data to d_data,
- * runs sk_frame there, copies SK and mask (and, if zero_flagged, the excised data) back, and
+ * runs sk_frame there, copies SK and mask (and, with SK_FRAME_ZERO_FLAGGED, the excised data) back, and
  * waits for the copies.  d_data (T*F*E bytes), d_SK, d_mask, workspace are caller-owned device
- * buffers; subset is a device pointer as above.  h_data is written only if zero_flagged. */
+ * buffers; subset is a device pointer as above.  h_data is written only with SK_FRAME_ZERO_FLAGGED;
+ * SK_FRAME_INPUTS_READY is ignored (the upload precedes the kernel). */
 int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
                   const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
-                  int zero_flagged, float* h_SK, uint8_t* h_mask,
+                  int flags, float* h_SK, uint8_t* h_mask,
                   uint8_t* d_data, float* d_SK, uint8_t* d_mask,
                   void* workspace, size_t workspace_bytes, void* stream);
 

@@ -162,8 +162,10 @@ def sk_flag(SK: torch.Tensor, M: int, N: int, n_sigma: float, sk_mean: float = 1
 def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: float = 3.0,
              sk_mean: float = 1.0, zero_flagged: bool = False, want_sums: bool = False,
              out: Optional[SKResult] = None, workspace: Optional[torch.Tensor] = None,
-             stream=None) -> SKResult:
-    """The fused path (one pass over HBM).  `data` is modified in place only if zero_flagged."""
+             stream=None, inputs_ready: bool = False) -> SKResult:
+    """The fused path (one pass over HBM).  `data` is modified in place only if zero_flagged.
+    inputs_ready = SK_FRAME_INPUTS_READY (include/sk_b200.h): `data`/`subset` are not written by
+    the work enqueued on the stream just before this call, so the kernel may overlap it."""
     _dev(data, torch.uint8, "data")
     T, F, E = data.shape
     B = T // M if M else 0
@@ -182,7 +184,8 @@ def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: flo
     if workspace is None:
         workspace = workspace_for(T, F, E, M, dev, st)
     _check(lib().sk_frame(data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
-                          int(bool(zero_flagged)), out.SK.data_ptr(), out.mask.data_ptr(),
+                          (1 if zero_flagged else 0) | (2 if inputs_ready else 0), out.SK.data_ptr(),
+                          out.mask.data_ptr(),
                           _ptr(out.S1), _ptr(out.S2), workspace.data_ptr(),
                           workspace.numel() * workspace.element_size(), st), "sk_frame")
     return out

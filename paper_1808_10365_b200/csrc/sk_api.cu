@@ -142,8 +142,18 @@ int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, cudaStrea
                              cudaSharedmemCarveoutMaxShared);
         attr_set = true;
     }
-    sk::sk_stream_kernel<L><<<dim3(p.slabs, p.F, p.B), 32, sk::kStreamSmemBytes, st>>>(tmap, p);
-    return SK_OK;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.slabs, p.F, p.B);
+    cfg.blockDim = dim3(32);
+    cfg.dynamicSmemBytes = sk::kStreamSmemBytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, sk::sk_stream_kernel<L>, tmap, p);
+    return e == cudaSuccess ? SK_OK : (int)e;
 }
 
 int launch_stream(int L, const sk::FrameParams& p, cudaStream_t st) {
@@ -157,15 +167,16 @@ int launch_stream(int L, const sk::FrameParams& p, cudaStream_t st) {
                                       gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    int rc;
     switch (L) {
-        case 16: launch_stream_L<16>(tmap, p, st); break;
-        case 8:  launch_stream_L<8>(tmap, p, st); break;
-        case 4:  launch_stream_L<4>(tmap, p, st); break;
-        case 2:  launch_stream_L<2>(tmap, p, st); break;
-        default: launch_stream_L<1>(tmap, p, st); break;
+        case 16: rc = launch_stream_L<16>(tmap, p, st); break;
+        case 8:  rc = launch_stream_L<8>(tmap, p, st); break;
+        case 4:  rc = launch_stream_L<4>(tmap, p, st); break;
+        case 2:  rc = launch_stream_L<2>(tmap, p, st); break;
+        default: rc = launch_stream_L<1>(tmap, p, st); break;
     }
-    ++g_launches;
-    return SK_OK;
+    if (rc == SK_OK) ++g_launches;
+    return rc;
 }
 
 int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
@@ -214,7 +225,7 @@ size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M) 
 
 static int frame_impl(const uint8_t* data, uint32_t T,
                       uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset, uint32_t first_n,
-                      float n_sigma, float sk_mean, float* SK, uint8_t* mask, uint32_t* S1o,
+                      float n_sigma, float sk_mean, int flags, float* SK, uint8_t* mask, uint32_t* S1o,
                       uint32_t* S2o, void* workspace, size_t workspace_bytes_given, cudaStream_t st) {
     if (!SK) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
@@ -227,6 +238,7 @@ static int frame_impl(const uint8_t* data, uint32_t T,
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
     p.subset = subset; p.first_n = subset ? 0 : first_n;
     p.n_sigma = n_sigma; p.sk_mean = sk_mean;
+    p.inputs_ready = (flags & SK_FRAME_INPUTS_READY) ? 1u : 0u;
     p.SK = SK; p.mask = mask; p.S1out = S1o; p.S2out = S2o;
     if (pl.vec) {
         const uint32_t cells = p.B * F;
@@ -294,12 +306,13 @@ int sk_flag(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, flo
 }
 
 int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
-             uint32_t first_n, float n_sigma, float sk_mean, int zero_flagged, float* SK, uint8_t* mask,
+             uint32_t first_n, float n_sigma, float sk_mean, int flags, float* SK, uint8_t* mask,
              uint32_t* S1_opt, uint32_t* S2_opt, void* workspace, size_t workspace_bytes_given,
              void* stream) {
+    const int zero_flagged = flags & SK_FRAME_ZERO_FLAGGED;
     if (!data || !SK || !mask) return SK_ERR_NULL;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = frame_impl(data, T, F, E, M, subset, first_n, n_sigma, sk_mean, SK, mask,
+    int rc = frame_impl(data, T, F, E, M, subset, first_n, n_sigma, sk_mean, flags, SK, mask,
                         S1_opt, S2_opt, workspace, workspace_bytes_given, st);
     if (rc != SK_OK || !zero_flagged) return rc;
     const uint32_t cells = (T / M) * F;
@@ -311,7 +324,7 @@ int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, cons
 }
 
 int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
-                  uint32_t first_n, float n_sigma, float sk_mean, int zero_flagged, float* h_SK,
+                  uint32_t first_n, float n_sigma, float sk_mean, int flags, float* h_SK,
                   uint8_t* h_mask, uint8_t* d_data, float* d_SK, uint8_t* d_mask, void* workspace,
                   size_t workspace_bytes_given, void* stream) {
     if (!h_data || !h_SK || !h_mask || !d_data || !d_SK || !d_mask) return SK_ERR_NULL;
@@ -320,6 +333,7 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
     const size_t bytes = (size_t)T * F * E, cells = (size_t)(T / M) * F;
     cudaError_t e = cudaMemcpyAsync(d_data, h_data, bytes, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return (int)e;
+    const int zero_flagged = flags & SK_FRAME_ZERO_FLAGGED;
     const int rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, zero_flagged, d_SK,
                             d_mask, nullptr, nullptr, workspace, workspace_bytes_given, stream);
     if (rc != SK_OK) return rc;

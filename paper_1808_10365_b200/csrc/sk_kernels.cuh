@@ -29,6 +29,7 @@ struct FrameParams {
     const uint32_t* S2in;
     double* partial;          // workspace: [cells][slabs]
     uint32_t* counter;        // workspace: [cells], zero on entry, zero on exit
+    uint32_t inputs_ready;    // stream kernel: read data before waiting for the previous grid
     uint32_t slabs;           // units per cell that are launched
     uint32_t nunits;          // cells * slabs
 };

@@ -80,6 +80,12 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
     const uint32_t full = p.M / R;                 // tiles with all R rows inside the block
     const uint32_t tiles = (p.M + R - 1) / R;
 
+    // Programmatic dependent launch: let the next grid on the stream start filling SM slots as
+    // they free up; wait for the previous grid before the first read unless the caller promised
+    // that nothing upstream writes our inputs (then only before the first write, below).
+    asm volatile("griddepcontrol.launch_dependents;");
+    if (!p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");
+
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * s, 1);
@@ -136,6 +142,8 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
             ++n;
         }
     }
+
+    if (p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");   // before the first write
 
     uint32_t S1[16], S2[16];
 #pragma unroll

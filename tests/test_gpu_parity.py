@@ -260,6 +260,39 @@ def test_deterministic_and_workspace_clean(sk, vector_path):
         assert torch.equal(a.mask, b.mask)
 
 
+def test_pipelined_frames_inputs_ready(sk, oracle):
+    """SK_FRAME_INPUTS_READY: back-to-back frames (distinct buffers, one shared workspace, one
+    stream) overlap through programmatic dependent launch; every frame's outputs must equal the
+    serialized call's bit for bit, and the first frames the oracle's."""
+    T, F, E, M = 2048, 2, 2048, 256
+    frames = [sk_synth.random_bytes(T, F, E, seed=100 + i).cuda() for i in range(8)]
+    ws = sk.workspace_for(T, F, E, M, frames[0].device, 4242)
+    serial = []
+    for d in frames:
+        serial.append(sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, workspace=ws, want_sums=True))
+        torch.cuda.synchronize()
+    for rep in range(3):
+        piped = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, workspace=ws, want_sums=True, inputs_ready=True)
+                 for d in frames]
+        torch.cuda.synchronize()
+        for a, b in zip(serial, piped):
+            assert torch.equal(a.SK.view(torch.int32), b.SK.view(torch.int32))
+            assert torch.equal(a.mask, b.mask)
+            assert torch.equal(a.S1.view(torch.int32), b.S1.view(torch.int32))
+            assert torch.equal(a.S2.view(torch.int32), b.S2.view(torch.int32))
+        assert int(ws.abs().sum().item()) == 0
+    # excision between pipelined frames: frame kernel -> excise kernel -> next frame's kernel
+    work = [d.clone() for d in frames[:4]]
+    outs = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, workspace=ws, zero_flagged=True, inputs_ready=True)
+            for d in work]
+    torch.cuda.synchronize()
+    for d0, d, o in zip(frames, work, outs):
+        ref = oracle.frame(d0.cpu().numpy(), M, n_sigma=2.0, sk_mean=0.4, zero_flagged=True)
+        np.testing.assert_array_equal(o.mask.cpu().numpy(), ref["mask"])
+        np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])
+        assert_sk_close(o.SK.cpu().numpy(), ref["SK"])
+
+
 def test_empty_subset_is_nan_and_flagged(sk):
     data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
     out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
