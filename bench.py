@@ -57,12 +57,36 @@ def peaks():
 
 
 def stored_traffic(cfg_name):
-    """dram bytes per launch from the committed ncu --set full capture, or None."""
+    """dram bytes per launch from the committed ncu --set full capture (profiles/), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
-            return json.load(f).get(cfg_name, {}).get("dram_bytes_per_launch")
+        import csv
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == cfg_name:
+                    return int(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
+
+
+def frame_ids(rank, nbuf):
+    """Frame numbers rank `rank` draws: disjoint between ranks (weak scaling, independent frames)."""
+    return [rank * 1000 + i for i in range(nbuf)]
+
+
+def max_over_ranks(x, world, device):
+    """A duration as the job sees it: the slowest rank's (no-op for one process)."""
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(samples_per_rank_step, world, steps, ms):
+    """Whole-job throughput: the samples all ranks processed / the slowest rank's time."""
+    return samples_per_rank_step * world * steps / (ms * 1e-3)
 
 
 class ClockSampler(threading.Thread):
@@ -193,7 +217,7 @@ def main():
     free = torch.cuda.mem_get_info()[0]
     nbuf = max(2, min(nbuf, int(free * 0.8) // frame_bytes))
     # every rank draws its own frames (weak scaling: independent frames per GPU, no collective)
-    bufs = [sk_synth.make_frame(cfg, device=dev, frame=rank * 1000 + i) for i in range(nbuf)]
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=fid) for fid in frame_ids(rank, nbuf)]
     null = sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * cfg.M), cw_block_inputs=None, cw_freqs=(),
                                          burst_fraction=0.0, sine_freqs=()), device=dev, frame=777)
     sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())     # null mean on 4-bit data
@@ -252,11 +276,7 @@ def main():
         e1.record(stream)
     barrier()
     sampler.window = (t_lo, time.perf_counter())
-    ms = e0.elapsed_time(e1)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
 
     # ---- end to end through the C ABI with host buffers (copies inside the timed region)
     Ke = args.e2e_steps or min(K, 20)
@@ -276,10 +296,7 @@ def main():
         e2e_step(i)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s = float(te.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     sampler.stop_flag = True
     sampler.join(timeout=2)
 
@@ -288,8 +305,7 @@ def main():
             dist.destroy_process_group()
         return
 
-    samples_per_step = frame_bytes * world
-    value = samples_per_step * K / (ms * 1e-3)
+    value = job_value(frame_bytes, world, K, ms)
     cells = cfg.B * cfg.F
     out_bytes = cells * 5
     flagged_bytes = int(flagged * frame_bytes) if args.zero else 0
@@ -311,7 +327,7 @@ def main():
                      "frac": achieved / peak, "traffic": stored_traffic(cfg.name), "peak_source": peak_src,
                      "frac_of_nominal_8000": achieved / 8000.0, "kernel": "sk_stream_kernel",
                      "algorithmic_bytes_per_launch": alg_bytes},
-        "e2e": {"value": frame_bytes * world * Ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": frame_bytes,
+        "e2e": {"value": job_value(frame_bytes, world, Ke, e2e_s * 1e3), "unit": UNIT, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": out_bytes, "steps": Ke, "api": "sk_frame_host (C ABI, pinned host buffers)"},
         "gpu_launches": int(launches),
         "clocks": sampler.summary(),

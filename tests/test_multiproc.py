@@ -1,0 +1,59 @@
+"""N > 1 host logic of bench.py on CPU: two processes, gloo backend, 127.0.0.1 rendezvous.
+The SK path shards by frames with no collective; what the ranks share is the
+timing protocol: disjoint frames per rank, max-over-ranks duration, whole-job throughput, and a
+reference arm that only rank 0 runs."""
+import os
+import socket
+import subprocess
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, torch.device("cpu"))     # rank 1 is slower
+    ids = bench.frame_ids(rank, 4)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, ids)
+    dist.barrier()
+    if rank == 0:
+        out.put((ms, gathered, bench.job_value(1000, world, 4, ms)))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_gloo():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    ms, ids, value = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert ms == 15.0                                         # the slowest rank's time
+    assert not set(ids[0]) & set(ids[1]) and len(ids[0]) == len(ids[1]) == 4
+    assert value == pytest.approx(1000 * 2 * 4 / 15e-3)       # all ranks' samples / that time
+
+
+def test_reference_arm_runs_on_rank0_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and r.stdout.strip() == ""
