@@ -3,6 +3,8 @@
 #include <atomic>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
+#include <cstring>
 
 #include "../../include/sk_b200.h"
 #include "sk_kernels.cuh"
@@ -22,18 +24,22 @@ inline int launch_status() {
 
 int sm_count();
 
-// Lanes per row for the vector path (slab width = 16*L inputs): a function of the shape (E and
-// the number of cells B*F) and of the device only, so that sk_combine and sk_frame split a cell
-// into the same units and add the float64 terms in the same order.  Wide 256-byte slabs when that
-// still gives every SM kWarpsWanted warps to run; otherwise narrower slabs (more, smaller units).
-constexpr uint32_t kWarpsWanted = 16;
-
-inline int lanes_per_row(uint32_t E, uint32_t cells, uint32_t M) {
+// Lanes per row for the vector path (slab width = 16*L inputs).  The sum over inputs follows a
+// canonical tree over the input indices (sk_kernels.cuh), so the choice affects speed only, never
+// a result: wide 256-byte slabs (fewest units, least per-unit work) when that still gives every
+// SM enough warps; otherwise narrower slabs.  A lone frame needs ~16 warps per SM of its own;
+// frames that overlap their neighbours on the stream (SK_FRAME_INPUTS_READY) share the SM with
+// them and run best on wide slabs from 8 warps per SM up (measured on config 1: 16.3 vs 17.0 us).
+inline int lanes_per_row(uint32_t E, uint32_t cells, uint32_t M, bool overlapped) {
     const uint32_t vecs = E / 16;            // 128-bit vectors per row
     int L = 16;
     while (L > 1 && (uint32_t)L > vecs) L >>= 1;
-    const unsigned long long want = (unsigned long long)sm_count() * kWarpsWanted;
+    const unsigned long long want = (unsigned long long)sm_count() * (overlapped ? 8u : 16u);
     while (L > 4 && (unsigned long long)cells * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
+    if (const char* e = std::getenv("SK_B200_LANES")) {     // tests: force a (narrower) slab width
+        const int v = std::atoi(e);
+        if (v >= 1 && v <= L && (v & (v - 1)) == 0) L = v;
+    }
     // long blocks: narrower slabs put more rows under one warp-wide read, so that a lane still
     // adds at most AccChain::kMaxSamples samples per unit (the stream kernel's exactness limit)
     while (L > 1 && (M + 32u / L - 1) / (32u / L) > sk::AccChain::kMaxSamples) L >>= 1;
@@ -64,12 +70,12 @@ struct Plan {
 };
 
 Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F, const uint8_t* subset,
-               uint32_t first_n, bool need_all_inputs) {
+               uint32_t first_n, bool need_all_inputs, bool overlapped) {
     Plan pl{};
     const uint32_t cells = B * F;
     pl.grid_ok = B <= 65535u && F <= 65535u;
     pl.vec = vector_ok(data, E);
-    pl.L = lanes_per_row(E, cells, M);
+    pl.L = lanes_per_row(E, cells, M, overlapped);
     const uint32_t W = 16u * pl.L;
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
@@ -208,7 +214,7 @@ int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint3
                   uint32_t* S1, uint32_t* S2, void* stream) {
     if (!data || !S1 || !S2) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
-    Plan pl = make_plan(data, E, M, T / M, F, nullptr, E, true);
+    Plan pl = make_plan(data, E, M, T / M, F, nullptr, E, true, false);
     if ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
@@ -232,7 +238,7 @@ static int frame_impl(const uint8_t* data, uint32_t T,
     if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
     if (mask && (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0)) return SK_ERR_PARAM;
     if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
-    Plan pl = make_plan(data, E, M, T / M, F, subset, first_n, S1o != nullptr);
+    Plan pl = make_plan(data, E, M, T / M, F, subset, first_n, S1o != nullptr, (flags & SK_FRAME_INPUTS_READY) != 0);
     if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
@@ -270,7 +276,7 @@ int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, u
     const bool vec = E % 16 == 0 &&
                      ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) == 0;
     if (vec) {
-        const int L = lanes_per_row(E, cells, M);
+        const int L = lanes_per_row(E, cells, M, false);
         p.slabs = (E + 16u * L - 1) / (16u * L);
         p.nunits = cells * p.slabs;
         const size_t smem = (size_t)p.slabs * sizeof(double);

@@ -6,8 +6,8 @@
 //           RPW-th row (RPW = 32/L rows are covered by one warp-wide 128-bit load).
 //   After the row loop the RPW row groups are summed with shuffles (integers: exact), each lane
 //   evaluates Eq. 11's term for its share of the 16 inputs in float64, the warp adds them with a
-//   fixed butterfly, and the unit's partial S2bar goes to the workspace.  The last unit of a cell
-//   to arrive (one atomic counter per cell) adds the partials in ascending slab order, evaluates
+//   canonical tree (below), and the unit's partial S2bar goes to the workspace.  The last unit of a
+//   cell to arrive (one atomic counter per cell) merges the partials in the same tree, evaluates
 //   Eq. 14, rounds to float32, takes the flag decision, and resets the counter.
 //   The order of every floating-point sum is fixed, so results are bit-reproducible.
 #pragma once
@@ -87,54 +87,158 @@ __device__ __forceinline__ int reduce_scatter_rows(uint32_t (&v1)[16], uint32_t 
     return base;
 }
 
-// a4 + a5 (within a unit): the unit's share of S2bar, identical on all lanes on return.
-// v1/v2[0..kOwned) are the sums of inputs e0+base .. ; `owner` is false for the duplicate lane
-// when RPW = 32.  Called by the fused kernel and by the combine kernel: same order in both.
+// ---- a5: the canonical order of the sum over inputs -------------------------------------------
+// S2bar = Tree(0, P), P = the power of two >= E, with
+//   Tree(lo, 1) = term of input lo (0.0 if lo >= E or the input is not selected),
+//   Tree(lo, n) = Tree(lo, n/2) + Tree(lo + n/2, n/2).
+// The order is a property of the input indices alone: it does not depend on the slab width, the
+// kernel, the launch flags or the SM count, so every path gives the same float64 S2bar (adding an
+// absent subtree's 0.0 is exact, and a + b = b + a).  A lane adds its aligned block pairwise, the
+// warp climbs the remaining levels of the unit's subtree with one xor-shuffle per level (the lane
+// bit that holds each input bit follows from reduce_scatter_rows), and the finalizer merges the
+// units' subtrees like a binary counter.
+
+// a4 + a5 within a unit: Tree(unit's first input, 16 L), identical on all lanes on return.
+// v1/v2[0..kOwned) are the sums of inputs e_first ..; `owner` is false for the duplicate lanes
+// when RPW = 32.  Called by both fused kernels and by the combine kernel.
 template <int L>
 __device__ __forceinline__ double unit_partial(const FrameParams& p, bool active, bool owner, uint32_t e_first,
                                                const uint32_t (&v1)[16], const uint32_t (&v2)[16]) {
+    constexpr int kOwn = Owned<L>::value;
+    constexpr int RPW = 32 / L;
     const double Md = (double)p.M, MM = __dmul_rn(Md, Md);
-    double part = 0.0;
+    // which of the lane's inputs are combined: decided once, so that the kOwn divisions below
+    // are straight-line code the scheduler can interleave
+    uint32_t sel = 0;
     if (active && owner) {
+        if (p.subset) {
 #pragma unroll
-        for (int i = 0; i < Owned<L>::value; ++i) {
-            const double t = eq11_term(Md, MM, v1[i], v2[i]);
-            part = __dadd_rn(part, selected(p, e_first + i) ? t : 0.0);
+            for (int i = 0; i < kOwn; ++i) sel |= (uint32_t)(__ldg(p.subset + e_first + i) != 0) << i;
+        } else {
+#pragma unroll
+            for (int i = 0; i < kOwn; ++i) sel |= (uint32_t)(e_first + i < p.first_n) << i;
         }
     }
-    return warp_sum_fixed(part);
+    double t[kOwn];
+#pragma unroll
+    for (int i = 0; i < kOwn; ++i) {
+        const double x = eq11_term(Md, MM, v1[i], v2[i]);
+        t[i] = ((sel >> i) & 1u) ? x : 0.0;
+    }
+#pragma unroll
+    for (int h = 1; h < kOwn; h *= 2)
+#pragma unroll
+        for (int i = 0; i + h < kOwn; i += 2 * h) t[i] = __dadd_rn(t[i], t[i + h]);
+    double x = t[0];
+    // input bits log2(kOwn) .. 3 live in the row-group bits of the lane, highest stage first
+#pragma unroll
+    for (int o = 16; o >= L; o >>= 1)
+        if (o < 32 && (RPW <= 16 || o < 16)) x = __dadd_rn(x, __shfl_xor_sync(0xffffffffu, x, o));
+    // input bits 4 .. live in the column bits of the lane
+#pragma unroll
+    for (int o = 1; o < L; o <<= 1) x = __dadd_rn(x, __shfl_xor_sync(0xffffffffu, x, o));
+    if (RPW == 32) x = __dadd_rn(x, __shfl_xor_sync(0xffffffffu, x, 16));   // duplicates hold 0.0
+    return x;
 }
 
-// a5 (across units, ascending slab order) + a6 + a7 for one cell; whole warp calls, lane 0 writes.
-__device__ __forceinline__ void finalize_cell(const FrameParams& p, uint32_t cell, int lane,
-                                              const volatile double* partials) {
+// a5 across units: merge equal-sized subtrees in index order, like a binary counter: neighbours
+// are added as soon as both exist; what is left at the end is folded from the smallest up (its
+// missing siblings are absent inputs, i.e. 0.0).  Slots are indexed by unrolled constants only,
+// so they stay in registers.
+struct TreeMerge {
+    static constexpr int kLevels = 20;
+    double v[kLevels];
+    uint32_t n = 0;                                 // subtrees pushed so far
+    __device__ __forceinline__ void push(double x) {
+        const uint32_t k = n++;
+        bool placed = false;
+#pragma unroll
+        for (int l = 0; l < kLevels; ++l) {
+            if (!placed) {
+                if ((k >> l) & 1u) x = __dadd_rn(v[l], x);
+                else { v[l] = x; placed = true; }
+            }
+        }
+    }
+    __device__ __forceinline__ double total() const {
+        double x = 0.0;
+        bool have = false;
+#pragma unroll
+        for (int l = 0; l < kLevels; ++l) {
+            if ((n >> l) & 1u) {
+                x = have ? __dadd_rn(v[l], x) : v[l];
+                have = true;
+            }
+        }
+        return x;
+    }
+};
+
+// A unit's partial travels through the workspace without any fence: the slot is written by one
+// relaxed 64-bit store whose bit pattern is never zero (a partial of +0.0 is stored as -0.0, which
+// adds like 0.0), and the finalizer polls a slot until it is non-zero.  The arrival counter only
+// elects the finalizer; it does not have to be ordered against the stores.
+__device__ __forceinline__ void store_partial(double* slot, double x) {
+    unsigned long long bits = (unsigned long long)__double_as_longlong(x);
+    if (bits == 0ull) bits = 0x8000000000000000ull;
+    asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(slot), "l"(bits) : "memory");
+}
+__device__ __forceinline__ double poll_partial(const double* slot) {
+    unsigned long long bits;
+    do {
+        asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(bits) : "l"(slot) : "memory");
+    } while (bits == 0ull);
+    return __longlong_as_double((long long)bits);
+}
+
+// a5 (across units) + a6 + a7 for one cell; whole warp calls, lane 0 writes.  32 units at a time:
+// an aligned group of 32 subtrees is summed with the canonical butterfly, groups are merged.
+// POLL: the partials are workspace slots that may still be in flight (fused kernels); otherwise
+// they are plain memory that is already complete (combine kernel: shared memory).
+template <bool POLL>
+__device__ __forceinline__ void finalize_cell(const FrameParams& p, uint32_t cell, int lane, const double* partials) {
     const uint32_t N = count_receivers(p, lane);
+    auto load = [&](uint32_t s) -> double {
+        if (s >= p.slabs) return 0.0;
+        return POLL ? poll_partial(partials + s) : partials[s];
+    };
+    double S2bar = load(lane);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) S2bar = __dadd_rn(S2bar, __shfl_xor_sync(0xffffffffu, S2bar, o));
+    if (p.slabs > 32) {                             // more than one group of 32 units: merge groups
+        TreeMerge tm;
+        tm.push(S2bar);
+        for (uint32_t s0 = 32; s0 < p.slabs; s0 += 32) {
+            double x = load(s0 + lane);
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) x = __dadd_rn(x, __shfl_xor_sync(0xffffffffu, x, o));
+            tm.push(x);
+        }
+        S2bar = tm.total();
+    }
     if (lane == 0) {
         const double Md = (double)p.M;
-        double S2bar = 0.0;
-        for (uint32_t s = 0; s < p.slabs; ++s) S2bar = __dadd_rn(S2bar, partials[s]);
         const float sk = eq14_sk(S2bar, Md, (double)N);
         p.SK[cell] = sk;
         if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, (double)N));
     }
 }
 
-// Fused kernel: publish the unit's partial; the last unit of the cell to arrive finalizes it.
+// Fused kernels: publish the unit's partial; the last unit of the cell to arrive finalizes it.
 __device__ __forceinline__ void publish_and_finalize(const FrameParams& p, uint32_t cell, uint32_t slab,
                                                      int lane, double part) {
+    double* slots = p.partial + (size_t)cell * p.slabs;
     uint32_t last = 0;
     if (lane == 0) {
-        p.partial[(size_t)cell * p.slabs + slab] = part;
-        __threadfence();
+        store_partial(slots + slab, part);
         last = (atomicAdd(p.counter + cell, 1u) == p.slabs - 1u);
     }
     last = __shfl_sync(0xffffffffu, last, 0);
     if (!last) return;
-    __threadfence();
-    finalize_cell(p, cell, lane, p.partial + (size_t)cell * p.slabs);
+    finalize_cell<true>(p, cell, lane, slots);
     __syncwarp();
     // leave the workspace all-zero: partials and counter (header contract)
-    for (uint32_t s = lane; s < p.slabs; s += 32) p.partial[(size_t)cell * p.slabs + s] = 0.0;
+    for (uint32_t s = lane; s < p.slabs; s += 32) slots[s] = 0.0;
     if (lane == 0) p.counter[cell] = 0u;
 }
 
@@ -244,12 +348,13 @@ sk_combine_kernel(const FrameParams p) {
         if (lane == 0) partials[slab] = part;
     }
     __syncthreads();
-    if (warp == 0) finalize_cell(p, cell, lane, partials);
+    if (warp == 0) finalize_cell<false>(p, cell, lane, partials);
 }
 
 // ------------------------------------------------------------- scalar fallback (any E, alignment)
-// One CTA per cell; thread t owns inputs t, t+256, ...; float64 terms are added per thread in
-// ascending e, then across threads with a fixed shared-memory tree.
+// One CTA per cell.  Inputs are taken 256 at a time (thread t owns input 256 c + t); a chunk's
+// terms are added with the canonical adjacent-first tree in shared memory, chunks are merged by
+// thread 0: the same S2bar as the vector kernels, bit for bit.
 constexpr int kScalarThreads = 256;
 
 __global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const FrameParams p) {
@@ -257,46 +362,55 @@ __global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const Fr
     __shared__ uint32_t cnt[kScalarThreads];
     const uint32_t cell = blockIdx.x;
     const uint32_t b = cell / p.F, f = cell % p.F;
-    const double Md = (double)p.M;
-    double part = 0.0;
+    const double Md = (double)p.M, MM = __dmul_rn(Md, Md);
+    TreeMerge tm;
     uint32_t nsel = 0;
-    for (uint32_t e = threadIdx.x; e < p.E; e += kScalarThreads) {
-        uint32_t s1 = 0, s2 = 0;
-        if (p.S1in) {
-            s1 = p.S1in[(size_t)cell * p.E + e];
-            s2 = p.S2in[(size_t)cell * p.E + e];
-        } else {
-            const uint8_t* q = p.data + ((size_t)b * p.M * p.F + f) * p.E + e;
-            const size_t rstride = (size_t)p.F * p.E;
-            for (uint32_t j = 0; j < p.M; ++j) {
-                const uint32_t pw = power_scalar(q[(size_t)j * rstride]);
-                s1 += pw;
-                s2 += pw * pw;
+    for (uint32_t c0 = 0; c0 < p.E; c0 += kScalarThreads) {
+        const uint32_t e = c0 + threadIdx.x;
+        double term = 0.0;
+        if (e < p.E) {
+            uint32_t s1 = 0, s2 = 0;
+            if (p.S1in) {
+                s1 = p.S1in[(size_t)cell * p.E + e];
+                s2 = p.S2in[(size_t)cell * p.E + e];
+            } else {
+                const uint8_t* q = p.data + ((size_t)b * p.M * p.F + f) * p.E + e;
+                const size_t rstride = (size_t)p.F * p.E;
+                for (uint32_t j = 0; j < p.M; ++j) {
+                    const uint32_t pw = power_scalar(q[(size_t)j * rstride]);
+                    s1 += pw;
+                    s2 += pw * pw;
+                }
+                if (p.S1out) {
+                    p.S1out[(size_t)cell * p.E + e] = s1;
+                    p.S2out[(size_t)cell * p.E + e] = s2;
+                }
             }
-            if (p.S1out) {
-                p.S1out[(size_t)cell * p.E + e] = s1;
-                p.S2out[(size_t)cell * p.E + e] = s2;
+            if (p.SK && selected(p, e)) {
+                term = eq11_term(Md, MM, s1, s2);
+                ++nsel;
             }
         }
-        if (p.SK && selected(p, e)) {
-            part = __dadd_rn(part, eq11_term(Md, __dmul_rn(Md, Md), s1, s2));
-            ++nsel;
+        if (!p.SK) continue;
+        red[threadIdx.x] = term;
+        __syncthreads();
+        for (int o = 1; o < kScalarThreads; o <<= 1) {
+            if ((threadIdx.x & (2 * o - 1)) == 0) red[threadIdx.x] = __dadd_rn(red[threadIdx.x], red[threadIdx.x + o]);
+            __syncthreads();
         }
+        if (threadIdx.x == 0) tm.push(red[0]);
+        __syncthreads();
     }
     if (!p.SK) return;
-    red[threadIdx.x] = part;
     cnt[threadIdx.x] = nsel;
     __syncthreads();
     for (int o = kScalarThreads / 2; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) {
-            red[threadIdx.x] = __dadd_rn(red[threadIdx.x], red[threadIdx.x + o]);
-            cnt[threadIdx.x] += cnt[threadIdx.x + o];
-        }
+        if ((int)threadIdx.x < o) cnt[threadIdx.x] += cnt[threadIdx.x + o];
         __syncthreads();
     }
     if (threadIdx.x == 0) {
         const double N = (double)cnt[0];
-        const float sk = eq14_sk(red[0], Md, N);
+        const float sk = eq14_sk(tm.total(), Md, N);
         p.SK[cell] = sk;
         if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, N));
     }

@@ -248,6 +248,34 @@ def test_vector_paths_bit_identical(sk, monkeypatch):
         assert torch.equal(a.mask, b.mask)
 
 
+def test_sk_independent_of_slab_width_and_kernel(sk, monkeypatch):
+    """The sum over inputs follows a canonical tree over the input indices: every slab width
+    (SK_B200_LANES), both vector kernels, the unfused path and the scalar kernel (misaligned
+    pointer) give the same SK bit for bit, receiver subsets and ragged E included."""
+    for (T, F, E, M) in [(512, 2, 2048, 128), (384, 3, 528, 96), (256, 1, 4096 + 48, 64)]:
+        data = sk_synth.random_bytes(T, F, E, seed=31)
+        data[:M, 0, :40] = 0x88
+        d = data.cuda()
+        flat = torch.empty(T * F * E + 1, dtype=torch.uint8, device="cuda")
+        mis = flat[1:].view(T, F, E)
+        mis.copy_(d)
+        rng = np.random.default_rng(5)
+        sub = rng.random(E) < 0.6
+        for kw in ({}, {"first_n": E // 3 + 5}, {"subset": sub}):
+            ref = sk.sk_frame(mis, M, **kw).SK.clone()          # scalar kernel
+            S1, S2 = sk.sk_power_sums(d, M)
+            for lanes in ("16", "8", "4", "2", "1"):
+                monkeypatch.setenv("SK_B200_LANES", lanes)
+                for path in ("tma", "ldg"):
+                    monkeypatch.setenv("SK_B200_PATH", path)
+                    got = sk.sk_frame(d, M, **kw).SK
+                    assert torch.equal(got.view(torch.int32), ref.view(torch.int32)), (T, F, E, M, kw.keys(), lanes, path)
+                un = sk.sk_combine(S1, S2, M, **kw)
+                assert torch.equal(un.view(torch.int32), ref.view(torch.int32)), (lanes, "combine")
+            monkeypatch.delenv("SK_B200_LANES")
+            monkeypatch.delenv("SK_B200_PATH")
+
+
 def test_deterministic_and_workspace_clean(sk, vector_path):
     data = sk_synth.random_bytes(1024, 2, 2048, seed=9).cuda()
     ws = sk.workspace_for(1024, 2, 2048, 256, data.device, 12345)
