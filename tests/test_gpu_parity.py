@@ -136,6 +136,11 @@ def test_config1_full_frame(sk, oracle, vector_path):
     ref = oracle.frame(host.numpy(), cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
     assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
     np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    # the launch configuration bench.py times: back-to-back calls with SK_FRAME_INPUTS_READY
+    piped = [sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0, inputs_ready=True) for _ in range(4)]
+    torch.cuda.synchronize()
+    for o in piped:
+        assert torch.equal(o.SK.view(torch.int32), out.SK.view(torch.int32)) and torch.equal(o.mask, out.mask)
     out2 = sk.sk_frame(data, cfg.M, want_sums=True)
     np.testing.assert_array_equal(u32np(out2.S1), ref["S1"])
     np.testing.assert_array_equal(u32np(out2.S2), ref["S2"])
@@ -192,6 +197,36 @@ def test_config2_rfi_mix_sampled(sk, oracle):
     again = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)   # idempotent
     assert torch.equal(again.mask, out.mask)
     assert bool((again.SK[out.mask.bool()] == 0).all())
+
+
+def test_config4_streaming_sampled(sk, oracle):
+    """Config 4 at full size (8 GiB per frame) the way bench.py --workload cfg4 --zero runs it:
+    frames back to back on one stream with SK_FRAME_INPUTS_READY and in-place excision.  Sampled
+    cells against the oracle one by one; excision checked at full size with torch reductions."""
+    cfg = sk_synth.config(4)
+    free = torch.cuda.mem_get_info()[0]
+    if free < 3 * cfg.nbytes + (4 << 30):
+        pytest.skip("needs ~28 GiB of free device memory")
+    frames = [sk_synth.make_frame(cfg, device="cuda", frame=i) for i in range(2)]
+    null = sk_synth.make_frame(cfg.with_(T=4 * cfg.M, cw_freqs=(), burst_fraction=0.0, sine_freqs=()),
+                               device="cuda", frame=3)
+    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())
+    before = frames[1].clone()
+    ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, frames[0].device, 77)
+    outs = [sk.sk_frame(d, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True, inputs_ready=True, workspace=ws)
+            for d in frames]
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(4)
+    cells = [(int(rng.integers(cfg.B)), int(rng.integers(cfg.F))) for _ in range(24)] + [(0, 0), (cfg.B - 1, cfg.F - 1)]
+    _check_sampled_cells(sk, oracle, before, outs[1], cfg.M, cells, 5.0, sk_mean)
+    mask = outs[1].mask.bool()
+    strong = sk_synth.rfi_cells(cfg, include_sine=False).cuda()
+    assert mask[strong].float().mean().item() > 0.99
+    assert 0.15 < mask.float().mean().item() < 0.30          # "20% RFI mix"
+    m = mask[:, None, :, None]
+    cellview = frames[1].view(cfg.B, cfg.M, cfg.F, cfg.E)
+    assert bool(((cellview == 0x88) | ~m).all())
+    assert bool(((cellview == before.view_as(cellview)) | m).all())
 
 
 def test_config3_sweep_sampled(sk, oracle):
