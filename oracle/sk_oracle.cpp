@@ -21,7 +21,8 @@
 //   A5  flag centre is the parameter sk_mean         A6  flag width sqrt(4/(M N))
 //   A7  strict '>' and NaN => flagged                A11 excision writes 0x88 to all E inputs
 //
-// Pins: tests/test_oracle_pins.py (all functions here are pinned).
+// Pins: tests/test_oracle_pins.py (all functions here are pinned, incl. sk_oracle_singles and
+// sk_oracle_significance of SURVEY.md section 8(f)).
 // Build: g++ -O2 -ffp-contract=off -shared -fPIC (oracle/build.py); no -ffast-math, no OpenMP.
 
 #include <cmath>
@@ -185,6 +186,30 @@ int sk_oracle_average_of_singles(const uint32_t* S1, const uint32_t* S2, uint32_
     return 0;
 }
 
+// Per-receiver estimates as an output (Eq. 8, the
+// "independent SK estimates" of PAPER.md:73, 145-151): SKi[b][f][e] = SK^_e rounded to float32.
+// A zero-power receiver gives 0 (reading A4).
+int sk_oracle_singles(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E,
+                      uint32_t M, float* SKi) {
+    if (!S1 || !S2 || !SKi || M < 2) return -1;
+    for (size_t i = 0; i < (size_t)B * F * E; ++i) {
+        const double s1 = (double)S1[i], s2 = (double)S2[i];
+        SKi[i] = (float)((s1 == 0.0) ? 0.0 : sk_oracle_single(s1, s2, (double)M));
+    }
+    return 0;
+}
+
+// Detection significance ("detection significance", the distance from the expected
+// mean in units of the expected spread): sig = (SK - sk_mean) / sqrt(4/(n N)) (Eq. 16), evaluated
+// in float64 from the float32 SK and rounded to float32.  |sig| > a is the flag of sk_oracle_flag.
+int sk_oracle_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N,
+                           float sk_mean, float* sig) {
+    if (!SK || !sig || M < 2 || N == 0) return -1;
+    const double sd = std::sqrt(4.0 / ((double)M * (double)N));
+    for (size_t c = 0; c < (size_t)B * F; ++c) sig[c] = (float)(((double)SK[c] - (double)sk_mean) / sd);
+    return 0;
+}
+
 // PAPER.md:97-99 Eq. 13 (first two lines), the un-rescaled multi-receiver estimator, and
 // PAPER.md:86 Eq. 10, S1bar = sum_i (S1)_i / mu_i (which must equal nN).
 int sk_oracle_eq13_and_s1bar(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F,
@@ -243,6 +268,6 @@ int sk_oracle_frame_float(const double* re, const double* im, uint32_t T, uint32
     return 0;
 }
 
-int sk_oracle_version(void) { return 1; }
+int sk_oracle_version(void) { return 2; }
 
 }  // extern "C"

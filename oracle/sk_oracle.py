@@ -107,6 +107,27 @@ def single(S1, S2, M):
     return lib().sk_oracle_single(float(S1), float(S2), float(M))
 
 
+def singles(S1, S2, M):
+    """PAPER.md:80 Eq. 8 per receiver as an output: float32 [B][F][E] (0 where S1 == 0)."""
+    S1 = np.ascontiguousarray(S1, dtype=np.uint32)
+    S2 = np.ascontiguousarray(S2, dtype=np.uint32)
+    B, F, E = S1.shape
+    out = np.empty((B, F, E), dtype=np.float32)
+    _check(lib().sk_oracle_singles(_p(S1, C.c_uint32), _p(S2, C.c_uint32), B, F, E, int(M), _p(out, C.c_float)),
+           "sk_oracle_singles")
+    return out
+
+
+def significance(SK, M, N, sk_mean=1.0):
+    """PAPER.md:183 detection significance: (SK - sk_mean) / sqrt(4/(M N)), float32 [B][F]."""
+    SK = np.ascontiguousarray(SK, dtype=np.float32)
+    B, F = SK.shape
+    out = np.empty((B, F), dtype=np.float32)
+    _check(lib().sk_oracle_significance(_p(SK, C.c_float), B, F, int(M), int(N), C.c_float(sk_mean),
+                                        _p(out, C.c_float)), "sk_oracle_significance")
+    return out
+
+
 def average_of_singles(S1, S2, M, subset=None, first_n=None):
     """PAPER.md:112 Eq. 14, third line: the mean of the per-receiver Eq. 8 estimates (float64)."""
     S1 = np.ascontiguousarray(S1, dtype=np.uint32)

@@ -119,6 +119,59 @@ def test_n1_reduces_to_single_receiver(oracle):
             assert sk[b, 0] == pytest.approx(oracle.single(S1[b, 0, e], S2[b, 0, e], M), rel=1e-14)
 
 
+def test_singles_output(oracle):
+    """NEXT-4: the per-receiver output is Eq. 8 element by element: the hand example's 0.625 and 0
+    (tests/golden/hand_example.txt), exact Fractions on random bytes, N = 1 combine, and its mean
+    over the receivers is Eq. 14 (PAPER.md:112 third line)."""
+    from fractions import Fraction
+    M = 4
+    data = np.array([[0x98, 0x99], [0x99, 0x99], [0x86, 0x99], [0x87, 0x99]], dtype=np.uint8).reshape(4, 1, 2)
+    S1, S2 = oracle.power_sums(data, M)
+    np.testing.assert_array_equal(oracle.singles(S1, S2, M)[0, 0], np.float32([0.625, 0.0]))
+    rng = np.random.default_rng(8)
+    M, E = 12, 7
+    data = rng.integers(0, 256, size=(2 * M, 2, E), dtype=np.uint8)
+    data[:M, 0, 3] = 0x88                                   # a dead receiver: 0 (reading A4)
+    S1, S2 = oracle.power_sums(data, M)
+    got = oracle.singles(S1, S2, M)
+    for b in range(2):
+        for f in range(2):
+            for e in range(E):
+                s1, s2 = int(S1[b, f, e]), int(S2[b, f, e])
+                want = Fraction(0) if s1 == 0 else Fraction(M + 1, M - 1) * (Fraction(M * s2, s1 * s1) - 1)
+                assert got[b, f, e] == np.float32(float(want))
+    assert got[0, 0, 3] == 0.0
+    sk64 = oracle.combine(S1, S2, M, want64=True)[1]
+    np.testing.assert_allclose(got.astype(np.float64).mean(axis=2), sk64, rtol=0, atol=2e-7)
+
+
+def test_significance(oracle):
+    """a value k spreads away from the mean has significance k; the flag at
+    threshold a is |significance| > a (same cells as oracle.flag away from the boundary)."""
+    M, N, mean = 256, 2048, 0.94
+    sd = np.sqrt(4.0 / (M * N))
+    k = np.array([[-7.5, -3.0, -0.25, 0.0, 0.5, 2.999, 3.001, 12.0]])
+    SK = (mean + k * sd).astype(np.float32)
+    sig = oracle.significance(SK, M, N, sk_mean=mean)
+    np.testing.assert_allclose(sig, k, rtol=0, atol=2e-4)          # float32 SK carries ~1e-4 sigma
+    assert np.array_equal(np.abs(sig) > 3.0, oracle.flag(SK, M, N, 3.0, sk_mean=mean).astype(bool))
+    assert np.isnan(oracle.significance(np.float32([[np.nan]]), M, N)[0, 0])
+
+
+def test_integration_lengths_from_sums(oracle):
+    """NEXT-2 ("a variety of integration lengths"): Eq. 7's sums over a block of
+    k*M samples are the sums of its k sub-blocks, so S1, S2 at M re-binned by k equal S1, S2
+    computed at k*M from the data: exact integers."""
+    rng = np.random.default_rng(9)
+    M, F, E = 8, 2, 5
+    data = rng.integers(0, 256, size=(12 * M, F, E), dtype=np.uint8)
+    S1, S2 = oracle.power_sums(data, M)
+    for k in (2, 3, 4, 6):
+        T1, T2 = oracle.power_sums(data, k * M)
+        np.testing.assert_array_equal(S1.reshape(12 // k, k, F, E).sum(axis=1, dtype=np.uint64), T1)
+        np.testing.assert_array_equal(S2.reshape(12 // k, k, F, E).sum(axis=1, dtype=np.uint64), T2)
+
+
 def test_two_level_closed_form(oracle):
     """A receiver alternating between powers a and b has M S2/S1^2 = 2(a^2+b^2)/(a+b)^2:
     with a=1 (0x98), b=4 (0xA8): 2*17/25 = 1.36, SK = (M+1)/(M-1)*0.36."""
