@@ -105,6 +105,28 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
                   uint8_t* d_data, float* d_SK, uint8_t* d_mask,
                   void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- outputs next to the hot path ---------------------------------- */
+
+/* Several integration lengths from one pass ("a variety of integration
+ * lengths"): Eq. 7's sums over factor*M samples are the sums of `factor` adjacent M-sample blocks.
+ * Reads S1, S2 [B][F][E] (from sk_power_sums or sk_frame's S1_opt/S2_opt); writes S1out, S2out
+ * [B/factor][F][E], exact integers, which sk_combine / sk_single then take with M*factor.
+ * B % factor == 0, factor >= 1, M*factor <= 65536 (the sums must still fit 32 bits). */
+int sk_rebin_sums(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E,
+                  uint32_t M, uint32_t factor, uint32_t* S1out, uint32_t* S2out, void* stream);
+
+/* Per-receiver estimates (Eq. 8; the "independent SK estimates" of PAPER.md:73):
+ * SKi[b][f][e] = (M+1)/(M-1) * (M S2/S1^2 - 1), float64 inside, float32 out; 0 where S1 == 0.
+ * Their mean over the combined receivers is sk_combine's SK (Eq. 14, third line). */
+int sk_single(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
+              float* SKi, void* stream);
+
+/* Detection significance: sig = (SK - sk_mean) / sqrt(4/(M N)) (Eq. 16), float64
+ * inside, float32 out; NaN stays NaN.  sk_flag's mask is |sig| > n_sigma up to float32 rounding
+ * at the boundary (the mask itself is always decided as the header's conventions state). */
+int sk_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, float sk_mean,
+                    float* sig, void* stream);
+
 /* Text for a return value of the calls above (static storage; never NULL). */
 const char* sk_strerror(int code);
 

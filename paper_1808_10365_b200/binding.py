@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
-           "sk_frame_host", "sk_strerror", "sk_version", "sk_launch_count")
+           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_strerror", "sk_version",
+           "sk_launch_count")
 
 _lib = None
 
@@ -40,11 +41,15 @@ def lib() -> C.CDLL:
     L.sk_frame_workspace_bytes.restype = sz
     L.sk_frame.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, sz, vp]
     L.sk_frame_host.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
+    L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
+    L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
     L.sk_strerror.argtypes = [i32]
     L.sk_strerror.restype = C.c_char_p
     L.sk_version.restype = i32
     L.sk_launch_count.restype = C.c_ulonglong
-    for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host"):
+    for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host", "sk_rebin_sums",
+                 "sk_single", "sk_significance"):
         getattr(L, name).restype = i32
     _lib = L
     return L
@@ -157,6 +162,39 @@ def sk_flag(SK: torch.Tensor, M: int, N: int, n_sigma: float, sk_mean: float = 1
     _check(lib().sk_flag(SK.data_ptr(), B, F, M, N, n_sigma, sk_mean, mask.data_ptr(), _stream(stream)),
            "sk_flag")
     return mask
+
+
+def sk_rebin_sums(S1: torch.Tensor, S2: torch.Tensor, M: int, factor: int, stream=None):
+    """sums at block length M re-binned to M*factor.  [B][F][E] -> [B/factor][F][E]."""
+    _dev(S1, torch.uint32, "S1")
+    _dev(S2, torch.uint32, "S2")
+    B, F, E = S1.shape
+    Bo = B // factor if factor else 0
+    O1 = torch.empty((Bo, F, E), dtype=torch.uint32, device=S1.device)
+    O2 = torch.empty_like(O1)
+    _check(lib().sk_rebin_sums(S1.data_ptr(), S2.data_ptr(), B, F, E, M, factor, O1.data_ptr(), O2.data_ptr(),
+                               _stream(stream)), "sk_rebin_sums")
+    return O1, O2
+
+
+def sk_single(S1: torch.Tensor, S2: torch.Tensor, M: int, stream=None):
+    """PAPER.md:80 Eq. 8 per receiver.  S1, S2 uint32 [B][F][E] -> SKi float32 [B][F][E]."""
+    _dev(S1, torch.uint32, "S1")
+    _dev(S2, torch.uint32, "S2")
+    B, F, E = S1.shape
+    SKi = torch.empty((B, F, E), dtype=torch.float32, device=S1.device)
+    _check(lib().sk_single(S1.data_ptr(), S2.data_ptr(), B, F, E, M, SKi.data_ptr(), _stream(stream)), "sk_single")
+    return SKi
+
+
+def sk_significance(SK: torch.Tensor, M: int, N: int, sk_mean: float = 1.0, stream=None):
+    """PAPER.md:183 detection significance.  SK float32 [B][F] -> float32 [B][F]."""
+    _dev(SK, torch.float32, "SK")
+    B, F = SK.shape
+    sig = torch.empty((B, F), dtype=torch.float32, device=SK.device)
+    _check(lib().sk_significance(SK.data_ptr(), B, F, M, N, sk_mean, sig.data_ptr(), _stream(stream)),
+           "sk_significance")
+    return sig
 
 
 def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: float = 3.0,

@@ -351,6 +351,54 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
     return e == cudaSuccess ? SK_OK : (int)e;
 }
 
+int sk_rebin_sums(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
+                  uint32_t factor, uint32_t* S1out, uint32_t* S2out, void* stream) {
+    if (!S1 || !S2 || !S1out || !S2out) return SK_ERR_NULL;
+    if (M < 2 || factor == 0 || (unsigned long long)M * factor > 65536ull) return SK_ERR_M;
+    if (B == 0 || F == 0 || E == 0 || B % factor != 0 || B / factor > 65535u) return SK_ERR_SHAPE;
+    const size_t FE = (size_t)F * E;
+    const uintptr_t al = reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2) |
+                         reinterpret_cast<uintptr_t>(S1out) | reinterpret_cast<uintptr_t>(S2out);
+    const bool vec = FE % 4 == 0 && (al & 15u) == 0;
+    const size_t per = vec ? FE / 4 : FE;
+    if ((per + 255) / 256 > 0x7fffffffull) return SK_ERR_SHAPE;
+    const dim3 grid((unsigned)((per + 255) / 256), B / factor);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (vec) sk::sk_rebin_kernel<true><<<grid, 256, 0, st>>>(S1, S2, S1out, S2out, FE, factor);
+    else     sk::sk_rebin_kernel<false><<<grid, 256, 0, st>>>(S1, S2, S1out, S2out, FE, factor);
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_single(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
+              float* SKi, void* stream) {
+    if (!S1 || !S2 || !SKi) return SK_ERR_NULL;
+    if (M < 2 || M > 65536) return SK_ERR_M;
+    if (B == 0 || F == 0 || E == 0) return SK_ERR_SHAPE;
+    const size_t n = (size_t)B * F * E;
+    if ((n + 255) / 256 > 0x7fffffffull) return SK_ERR_SHAPE;
+    const double Md = (double)M;
+    sk::sk_single_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(S1, S2, SKi, n, Md,
+                                                                                       (Md + 1.0) / (Md - 1.0));
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, float sk_mean, float* sig,
+                    void* stream) {
+    if (!SK || !sig) return SK_ERR_NULL;
+    if (M < 2 || M > 65536) return SK_ERR_M;
+    if (B == 0 || F == 0 || (unsigned long long)B * F >= (1ull << 31)) return SK_ERR_SHAPE;
+    if (N == 0) return SK_ERR_N;
+    if (!std::isfinite(sk_mean)) return SK_ERR_PARAM;
+    const size_t cells = (size_t)B * F;
+    const double sd = std::sqrt(4.0 / ((double)M * (double)N));
+    sk::sk_significance_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        SK, sig, cells, (double)sk_mean, sd);
+    ++g_launches;
+    return launch_status();
+}
+
 const char* sk_strerror(int code) {
     switch (code) {
         case SK_OK: return "ok";
@@ -364,7 +412,7 @@ const char* sk_strerror(int code) {
     }
 }
 
-int sk_version(void) { return 100; }
+int sk_version(void) { return 101; }
 
 unsigned long long sk_launch_count(void) { return g_launches.load(); }
 

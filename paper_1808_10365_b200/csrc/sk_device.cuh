@@ -197,7 +197,8 @@ __device__ __forceinline__ double u32_to_f64(uint32_t u) {
     return __dsub_rn(__hiloint2double(0x43300000, (int)u), 4503599627370496.0);
 }
 
-// n / y for 1 <= y < 2^53, 0 <= n < 2^60: hardware reciprocal seed, two Newton steps, one
+// n / y for finite n >= 0 and positive normal y (here 1 <= y < 2^53, n < 2^60, and the flag
+// spread sqrt(4/(M N))): hardware reciprocal seed, two Newton steps, one
 // correction of the quotient.  Branch-free; the result is within one ulp of n / y (normally the
 // correctly rounded quotient).  Every kernel divides through this one function, so all paths
 // agree bit for bit; against the oracle's IEEE division the difference is <= 2.2e-16 relative

@@ -423,6 +423,62 @@ __global__ void sk_flag_kernel(const float* __restrict__ SK, uint8_t* __restrict
     if (i < cells) mask[i] = flag_decision(SK[i], sk_mean, thr);
 }
 
+// ------------------------------------------------------------------ SURVEY 8(f) NEXT-2 / NEXT-4
+// Re-binned sums ("a variety of integration lengths"): Eq. 7 over k*M samples is
+// the sum of k adjacent M-sample blocks.  in [B][FE] -> out [B/k][FE]; VEC: 4 inputs per thread.
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+sk_rebin_kernel(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ A2, uint32_t* __restrict__ O1,
+                uint32_t* __restrict__ O2, size_t FE, uint32_t k) {
+    const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * (VEC ? 4 : 1);
+    if (i >= FE) return;
+    const size_t bo = blockIdx.y;
+    const uint32_t* p1 = A1 + bo * k * FE + i;
+    const uint32_t* p2 = A2 + bo * k * FE + i;
+    if (VEC) {
+        uint4 s1 = make_uint4(0, 0, 0, 0), s2 = s1;
+        for (uint32_t j = 0; j < k; ++j) {
+            const uint4 a = __ldg(reinterpret_cast<const uint4*>(p1 + (size_t)j * FE));
+            const uint4 b = __ldg(reinterpret_cast<const uint4*>(p2 + (size_t)j * FE));
+            s1.x += a.x; s1.y += a.y; s1.z += a.z; s1.w += a.w;
+            s2.x += b.x; s2.y += b.y; s2.z += b.z; s2.w += b.w;
+        }
+        *reinterpret_cast<uint4*>(O1 + bo * FE + i) = s1;
+        *reinterpret_cast<uint4*>(O2 + bo * FE + i) = s2;
+    } else {
+        uint32_t s1 = 0, s2 = 0;
+        for (uint32_t j = 0; j < k; ++j) { s1 += __ldg(p1 + (size_t)j * FE); s2 += __ldg(p2 + (size_t)j * FE); }
+        O1[bo * FE + i] = s1;
+        O2[bo * FE + i] = s2;
+    }
+}
+
+// Per-receiver estimate (Eq. 8): SKi = (M+1)/(M-1) * (M S2 / S1^2 - 1) in float64,
+// rounded to float32; a zero-power receiver gives 0 (A4).  `a` = (M+1)/(M-1) from the host.
+__global__ void __launch_bounds__(256)
+sk_single_kernel(const uint32_t* __restrict__ S1, const uint32_t* __restrict__ S2, float* __restrict__ SKi,
+                 size_t n, double M, double a) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t u1 = __ldg(S1 + i);
+    const double s1 = u32_to_f64(u1), s2 = u32_to_f64(__ldg(S2 + i));
+    const double q = div_f64(__dmul_rn(M, s2), __dmul_rn(s1, s1));
+    const double v = __dmul_rn(a, __dsub_rn(q, 1.0));
+    SKi[i] = u1 == 0u ? 0.0f : __double2float_rn(v);
+}
+
+// Detection significance: (SK - sk_mean) / sd, sd = sqrt(4/(M N)) from the host.
+__global__ void sk_significance_kernel(const float* __restrict__ SK, float* __restrict__ sig, size_t cells,
+                                       double sk_mean, double sd) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cells) return;
+    const double d = __dsub_rn((double)SK[i], sk_mean);
+    // div_f64 wants a positive divisor and a finite non-negative dividend: divide |d|, restore the sign
+    const double q = div_f64(fabs(d), sd);
+    sig[i] = (d != d || fabs(d) == __longlong_as_double(0x7ff0000000000000ll))
+                 ? __double2float_rn(d) : __double2float_rn(d < 0.0 ? -q : q);
+}
+
 // ------------------------------------------------------------------------------------- a8
 // Excision: every byte of every flagged cell becomes 0x88 (the encoded 0+0i).
 // grid = (cells, row chunks); a CTA whose cell is clean exits at once.

@@ -356,6 +356,56 @@ def test_pipelined_frames_inputs_ready(sk, oracle):
         assert_sk_close(o.SK.cpu().numpy(), ref["SK"])
 
 
+@pytest.mark.parametrize("T,F,E,M", [(768, 2, 272, 32), (1536, 1, 2048, 64), (480, 3, 37, 20)])
+def test_integration_lengths_from_one_pass(sk, oracle, T, F, E, M):
+    """S1, S2 of one pass at M, re-binned on the device by
+    k, equal the oracle's sums at k*M bit for bit, and SK / mask from them equal the oracle's at k*M."""
+    data = sk_synth.random_bytes(T, F, E, seed=41)
+    d = data.cuda()
+    base = sk.sk_frame(d, M, want_sums=True)
+    B = T // M
+    for k in (1, 2, 3, 4, 6, 12):
+        if B % k:
+            continue
+        R1, R2 = sk.sk_rebin_sums(base.S1, base.S2, M, k)
+        ref = oracle.frame(data.numpy(), M * k, n_sigma=2.0, sk_mean=0.4)
+        np.testing.assert_array_equal(u32np(R1), ref["S1"])
+        np.testing.assert_array_equal(u32np(R2), ref["S2"])
+        SK = sk.sk_combine(R1, R2, M * k)
+        assert_sk_close(SK.cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(sk.sk_flag(SK, M * k, E, 2.0, 0.4).cpu().numpy(), ref["mask"])
+        direct = sk.sk_frame(d, M * k, n_sigma=2.0, sk_mean=0.4)        # one pass at k*M: same bits
+        assert torch.equal(direct.SK.view(torch.int32), SK.view(torch.int32))
+    with pytest.raises(sk.SKError):
+        sk.sk_rebin_sums(base.S1, base.S2, M, 5 if B % 5 else 7)
+
+
+@pytest.mark.parametrize("T,F,E,M", [(512, 2, 272, 256), (640, 1, 2048, 64), (300, 3, 37, 100)])
+def test_per_receiver_sk_and_significance(sk, oracle, T, F, E, M):
+    """Eq. 8 per receiver and the detection significance, against the oracle
+    element by element (1e-6 relative); the mean of the per-receiver values is Eq. 14's SK."""
+    data = sk_synth.random_bytes(T, F, E, seed=43)
+    data[:M, 0, :5] = 0x88                                  # dead receivers: exactly 0
+    d = data.cuda()
+    out = sk.sk_frame(d, M, n_sigma=3.0, sk_mean=0.4, want_sums=True)
+    S1, S2 = u32np(out.S1), u32np(out.S2)
+    SKi = sk.sk_single(out.S1, out.S2, M).cpu().numpy()
+    ref = oracle.singles(S1, S2, M)
+    assert_sk_close(SKi, ref)
+    assert (SKi[0, 0, :5] == 0).all()
+    np.testing.assert_allclose(SKi.astype(np.float64).mean(axis=2), out.SK.cpu().numpy(), rtol=0, atol=5e-7 * E ** 0.5)
+    SK = out.SK.clone()
+    SK[0, 0] = float("nan")
+    sig = sk.sk_significance(SK, M, E, 0.4).cpu().numpy()
+    rs = oracle.significance(SK.cpu().numpy(), M, E, 0.4)
+    assert np.isnan(sig[0, 0]) and np.isnan(rs[0, 0])
+    ok = ~np.isnan(rs)
+    assert_sk_close(sig[ok], rs[ok])
+    far = ok & (np.abs(np.abs(rs) - 3.0) > 1e-3)            # away from the boundary: the flag itself
+    m = sk.sk_flag(SK, M, E, 3.0, 0.4).cpu().numpy().astype(bool)
+    assert np.array_equal((np.abs(sig) > 3.0)[far], m[far])
+
+
 def test_empty_subset_is_nan_and_flagged(sk):
     data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
     out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
