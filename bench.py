@@ -35,6 +35,9 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
+    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single"],
+                    help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
+                         "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -186,10 +189,54 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_aux(args):
+    """--op rebin|single: one of the small HBM-bound kernels beside the hot path, on S1/S2 arrays of
+    config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), two rotating copies."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    torch.cuda.set_device(0)
+    cfg = sk_synth.config(2)
+    frame = sk_synth.make_frame(cfg, device="cuda")
+    S1, S2 = sk.sk_power_sums(frame, cfg.M)
+    del frame
+    reps = 8                                               # config 2's 2048 cells x 8 = config 4's 16384
+    sums = [(S1.repeat(reps, 1, 1), S2.repeat(reps, 1, 1)) for _ in range(2)]
+    B, F, E = sums[0][0].shape
+    n = B * F * E
+    fn = (lambda a, b: sk.sk_rebin_sums(a, b, cfg.M, 2)) if args.op == "rebin" else (lambda a, b: sk.sk_single(a, b, cfg.M))
+    alg = n * 8 + (n * 8 // 2 if args.op == "rebin" else n * 4)
+    K, W = args.steps if args.steps != 2000 else 50, max(args.warmup, 3)
+    for i in range(W):
+        fn(*sums[i % 2])
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = sk.sk_launch_count()
+    e0.record()
+    for i in range(K):
+        fn(*sums[i % 2])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    peak, peak_src = peaks()
+    print(json.dumps({
+        "op": args.op, "metric": "sums_elements_per_s", "value": n / (ms * 1e-3), "unit": "elements/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
+        "dtype": "u32" if args.op == "rebin" else "u32->f64->f32",
+        "config": {"workload": f"S1,S2 [{B}][{F}][{E}] uint32 (config 4's size), M={cfg.M}",
+                   "l2": "two rotating copies, 256 MiB each"},
+        "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": alg / (ms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg},
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.op != "frame":
+        return run_aux(args)
 
     import torch
     import torch.distributed as dist

@@ -376,10 +376,15 @@ int sk_single(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, ui
     if (M < 2 || M > 65536) return SK_ERR_M;
     if (B == 0 || F == 0 || E == 0) return SK_ERR_SHAPE;
     const size_t n = (size_t)B * F * E;
-    if ((n + 255) / 256 > 0x7fffffffull) return SK_ERR_SHAPE;
-    const double Md = (double)M;
-    sk::sk_single_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(S1, S2, SKi, n, Md,
-                                                                                       (Md + 1.0) / (Md - 1.0));
+    const uintptr_t al = reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2) |
+                         reinterpret_cast<uintptr_t>(SKi);
+    const bool vec = n % 4 == 0 && (al & 15u) == 0;
+    const size_t per = vec ? n / 4 : n;
+    if ((per + 255) / 256 > 0x7fffffffull) return SK_ERR_SHAPE;
+    const double Md = (double)M, a = (Md + 1.0) / (Md - 1.0);
+    const unsigned grid = (unsigned)((per + 255) / 256);
+    if (vec) sk::sk_single_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(S1, S2, SKi, n, Md, a);
+    else     sk::sk_single_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(S1, S2, SKi, n, Md, a);
     ++g_launches;
     return launch_status();
 }

@@ -206,12 +206,10 @@ __device__ __forceinline__ double u32_to_f64(uint32_t u) {
 __device__ __forceinline__ double div_f64(double n, double y) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
-    double e = __fma_rn(-y, r, 1.0);
-    r = __fma_rn(r, e, r);
+    double e = __fma_rn(-y, r, 1.0);               // seed: ~2^-20 relative (upper mantissa word only)
+    r = __fma_rn(r, e, r);                         // 2^-40
     e = __fma_rn(-y, r, 1.0);
-    r = __fma_rn(r, e, r);
-    e = __fma_rn(-y, r, 1.0);
-    r = __fma_rn(r, e, r);
+    r = __fma_rn(r, e, r);                         // 2^-80: r is the rounded reciprocal
     const double q = __dmul_rn(n, r);
     return __fma_rn(__fma_rn(-y, q, n), r, q);
 }

@@ -455,16 +455,26 @@ sk_rebin_kernel(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ A2
 
 // Per-receiver estimate (Eq. 8): SKi = (M+1)/(M-1) * (M S2 / S1^2 - 1) in float64,
 // rounded to float32; a zero-power receiver gives 0 (A4).  `a` = (M+1)/(M-1) from the host.
+__device__ __forceinline__ float eq8_single(uint32_t u1, uint32_t u2, double M, double a) {
+    const double s1 = u32_to_f64(u1), s2 = u32_to_f64(u2);
+    const double q = div_f64(__dmul_rn(M, s2), __dmul_rn(s1, s1));
+    return u1 == 0u ? 0.0f : __double2float_rn(__dmul_rn(a, __dsub_rn(q, 1.0)));
+}
+
+template <bool VEC>
 __global__ void __launch_bounds__(256)
 sk_single_kernel(const uint32_t* __restrict__ S1, const uint32_t* __restrict__ S2, float* __restrict__ SKi,
                  size_t n, double M, double a) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * (VEC ? 4 : 1);
     if (i >= n) return;
-    const uint32_t u1 = __ldg(S1 + i);
-    const double s1 = u32_to_f64(u1), s2 = u32_to_f64(__ldg(S2 + i));
-    const double q = div_f64(__dmul_rn(M, s2), __dmul_rn(s1, s1));
-    const double v = __dmul_rn(a, __dsub_rn(q, 1.0));
-    SKi[i] = u1 == 0u ? 0.0f : __double2float_rn(v);
+    if (VEC) {
+        const uint4 u1 = __ldg(reinterpret_cast<const uint4*>(S1 + i));
+        const uint4 u2 = __ldg(reinterpret_cast<const uint4*>(S2 + i));
+        *reinterpret_cast<float4*>(SKi + i) = make_float4(eq8_single(u1.x, u2.x, M, a), eq8_single(u1.y, u2.y, M, a),
+                                                          eq8_single(u1.z, u2.z, M, a), eq8_single(u1.w, u2.w, M, a));
+    } else {
+        SKi[i] = eq8_single(__ldg(S1 + i), __ldg(S2 + i), M, a);
+    }
 }
 
 // Detection significance: (SK - sk_mean) / sd, sd = sqrt(4/(M N)) from the host.

@@ -406,6 +406,21 @@ def test_per_receiver_sk_and_significance(sk, oracle, T, F, E, M):
     assert np.array_equal((np.abs(sig) > 3.0)[far], m[far])
 
 
+def test_constant_modulus_is_exactly_zero_on_device(sk):
+    """Pin P1 on the device: constant-modulus samples have M^2 S2 / S1^2 = M exactly, so the
+    quotient of div_f64 must be exact and SK, SKi come out as 0.0 exactly (no tolerance)."""
+    rng = np.random.default_rng(12)
+    vals = [(5, 0), (-5, 0), (0, 5), (0, -5), (3, 4), (-3, 4), (4, -3), (-4, -3)]
+    pick = rng.integers(0, len(vals), size=(768, 2, 272))
+    re = np.array([v[0] for v in vals])[pick]
+    im = np.array([v[1] for v in vals])[pick]
+    data = torch.from_numpy((((re + 8) << 4) | (im + 8)).astype(np.uint8)).cuda()
+    for M in (64, 96, 256):
+        out = sk.sk_frame(data, M, want_sums=True)
+        assert bool((out.SK == 0).all())
+        assert bool((sk.sk_single(out.S1, out.S2, M) == 0).all())
+
+
 def test_empty_subset_is_nan_and_flagged(sk):
     data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
     out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
