@@ -268,6 +268,82 @@ int sk_oracle_frame_float(const double* re, const double* im, uint32_t T, uint32
     return 0;
 }
 
-int sk_oracle_version(void) { return 2; }
+// ---------------------------------------------------------------------------------------------
+// the digitisation simulation of PAPER.md:276-284 (App. B).
+// "a set of sample data was generated which mimicked the properties of CHIME's intermediate data
+// products - 4+4-bit complex Gaussian data (bounded between -7 and 7) with an RMS of ~1.52
+// least-significant bits in each component."
+//
+// Random numbers: the counter-based generator Philox4x32-10 (Salmon, Moraes, Dror, Shaw, "Parallel
+// random numbers: as easy as 1, 2, 3", SC'11), restated here from the paper's description; the
+// CUDA path has its own copy.  Pinned by the published known-answer vectors (tests).
+static inline void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+int sk_oracle_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+    if (!ctr || !key || !out) return -1;
+    philox4x32_10(ctr, key, out);
+    return 0;
+}
+
+// One digitised component from one 32-bit uniform u and the receiver's 14 ascending thresholds
+// thr[j] = 2^32 * P(value <= j - 7) (the caller's model of round-and-clip to [-7, 7]):
+// value = -7 + #{ j : u >= thr[j] }.
+static inline int digitise(uint32_t u, const uint32_t* thr) {
+    int v = -7;
+    for (int j = 0; j < 14; ++j) v += (u >= thr[j]) ? 1 : 0;
+    return v;
+}
+
+// data[t][f][e]: for row r = t*F + f and receiver pair j = e/2 the generator is called with
+// counter (j, r, frame_lo, frame_hi) and key (seed_lo, seed_hi); words 0, 1 give (re, im) of
+// receiver 2j, words 2, 3 give (re, im) of receiver 2j+1.  byte = (re+8)<<4 | (im+8).
+int sk_oracle_sim_digitised(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, const uint32_t* thr,
+                            uint64_t seed, uint64_t frame) {
+    if (!data || !thr || T == 0 || F == 0 || E == 0) return -1;
+    if ((uint64_t)T * F > 0xFFFFFFFFull) return -1;
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    for (uint64_t r = 0; r < (uint64_t)T * F; ++r) {
+        for (uint32_t e = 0; e < E; ++e) {
+            const uint32_t ctr[4] = {e / 2, (uint32_t)r, (uint32_t)frame, (uint32_t)(frame >> 32)};
+            uint32_t w[4];
+            philox4x32_10(ctr, key, w);
+            const int re = digitise(w[2 * (e & 1)], thr + (size_t)e * 14);
+            const int im = digitise(w[2 * (e & 1) + 1], thr + (size_t)e * 14);
+            data[r * E + e] = (uint8_t)(((re + 8) << 4) | (im + 8));
+        }
+    }
+    return 0;
+}
+
+// Mean and unbiased variance of the estimates over the blocks, per frequency (the "statistics of
+// those estimates"): two passes in float64, NaN if B < 2 for the variance.
+int sk_oracle_moments(const float* SK, uint32_t B, uint32_t F, double* mean, double* var) {
+    if (!SK || !mean || !var || B == 0 || F == 0) return -1;
+    for (uint32_t f = 0; f < F; ++f) {
+        double m = 0.0;
+        for (uint32_t b = 0; b < B; ++b) m += (double)SK[(size_t)b * F + f];
+        m /= (double)B;
+        double v = 0.0;
+        for (uint32_t b = 0; b < B; ++b) {
+            const double d = (double)SK[(size_t)b * F + f] - m;
+            v += d * d;
+        }
+        mean[f] = m;
+        var[f] = (B > 1) ? v / (double)(B - 1) : std::nan("");
+    }
+    return 0;
+}
+
+int sk_oracle_version(void) { return 3; }
 
 }  // extern "C"

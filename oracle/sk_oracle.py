@@ -178,3 +178,34 @@ def frame_float(re, im, M, subset=None, first_n=None):
                                        _p(sub, C.c_uint8), int(first_n or 0), _p(SK, C.c_double),
                                        _p(S1, C.c_double), _p(S2, C.c_double)), "frame_float")
     return SK, S1, S2
+
+
+def philox(ctr, key):
+    """Philox4x32-10 (Salmon et al., SC'11): 4 counter words, 2 key words -> 4 output words."""
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    _check(lib().sk_oracle_philox(_p(ctr, C.c_uint32), _p(key, C.c_uint32), _p(out, C.c_uint32)), "sk_oracle_philox")
+    return out
+
+
+def sim_digitised(T, F, E, thr, seed, frame=0):
+    """PAPER.md:276-284 (App. B): seeded 4+4-bit round-and-clip Gaussian bytes [T][F][E] from the
+    per-receiver thresholds thr uint32 [E][14]."""
+    thr = np.ascontiguousarray(thr, dtype=np.uint32)
+    assert thr.shape == (E, 14)
+    data = np.empty((T, F, E), dtype=np.uint8)
+    _check(lib().sk_oracle_sim_digitised(_p(data, C.c_uint8), T, F, E, _p(thr, C.c_uint32),
+                                         C.c_uint64(seed), C.c_uint64(frame)), "sk_oracle_sim_digitised")
+    return data
+
+
+def moments(SK):
+    """Mean and unbiased variance of SK over the blocks, per frequency (float64 [F] each)."""
+    SK = np.ascontiguousarray(SK, dtype=np.float32)
+    B, F = SK.shape
+    mean = np.empty(F, dtype=np.float64)
+    var = np.empty(F, dtype=np.float64)
+    _check(lib().sk_oracle_moments(_p(SK, C.c_float), B, F, _p(mean, C.c_double), _p(var, C.c_double)),
+           "sk_oracle_moments")
+    return mean, var

@@ -259,3 +259,16 @@ def random_bytes(T: int, F: int, E: int, seed: int, device="cpu") -> torch.Tenso
     g = torch.Generator(device="cpu")
     g.manual_seed(seed)
     return torch.randint(0, 256, (T, F, E), generator=g, dtype=torch.uint8).to(device)
+
+
+def digitiser_thresholds(sigma) -> torch.Tensor:
+    """Input model of the App. B simulation (Gaussian components rounded to the
+    nearest level and bounded to [-7, 7]): for every receiver the 14 cumulative probabilities
+    P(round-and-clip(N(0, sigma_e^2)) <= j - 7) = Phi((j - 6.5) / sigma_e), j = 0..13, scaled to
+    32-bit thresholds.  uint32 [E][14] (stored as int64-safe numpy-compatible uint32 values).
+    Both the oracle's and the CUDA path's samplers take this table as an input."""
+    sig = torch.as_tensor(sigma, dtype=torch.float64).reshape(-1, 1)
+    edges = (torch.arange(14, dtype=torch.float64) - 6.5).reshape(1, -1)
+    cdf = torch.special.ndtr(edges / sig)
+    thr = torch.clamp(torch.floor(cdf * 4294967296.0), 0, 4294967295.0)
+    return thr.to(torch.int64).to(torch.uint32)

@@ -399,3 +399,96 @@ def test_bad_arguments(oracle):
         oracle.combine(S1, S2, 4, first_n=5)   # N > E
     with pytest.raises(ValueError):
         oracle.combine(S1, S2, 4, subset=[0, 0, 0, 0])   # N == 0
+
+
+# ---- App. B digitisation simulation ---------------------
+def _philox_py(ctr, key):
+    """Philox4x32-10 written out independently of the oracle (Salmon et al., SC'11, section 3.3):
+    ten rounds of two 32x32->64 multiplies by fixed constants, crossed with the key, which is
+    bumped by the Weyl constants every round."""
+    c = [int(x) for x in ctr]
+    k = [int(x) for x in key]
+    for _ in range(10):
+        p0, p1 = 0xD2511F53 * c[0], 0xCD9E8D57 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+        k = [(k[0] + 0x9E3779B9) & 0xFFFFFFFF, (k[1] + 0xBB67AE85) & 0xFFFFFFFF]
+    return c
+
+
+def test_philox_known_answers(oracle):
+    """The published known-answer vectors of Philox4x32-10 (Random123 distribution, kat_vectors:
+    zero counter and key; all-ones; the digits of pi)."""
+    kat = [
+        ([0, 0, 0, 0], [0, 0], [0x6627E8D5, 0xE169C58D, 0xBC57AC4C, 0x9B00DBD8]),
+        ([0xFFFFFFFF] * 4, [0xFFFFFFFF] * 2, [0x408F276D, 0x41C83B0E, 0xA20BC7C6, 0x6D5451FD]),
+        ([0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344], [0xA4093822, 0x299F31D0],
+         [0xD16CFE09, 0x94FDCCEB, 0x5001E420, 0x24126EA1]),
+    ]
+    for ctr, key, want in kat:
+        assert [int(x) for x in oracle.philox(ctr, key)] == want
+        assert _philox_py(ctr, key) == want
+
+
+def test_sim_digitised_layout_and_pmf(oracle):
+    """Counter layout and threshold rule element by element (independent Philox), then the
+    empirical distribution against the model's exact probabilities and RMS."""
+    import sk_synth
+    T, F, E = 6, 2, 5
+    sig = np.array([0.7, 1.52, 2.5, 3.5, 9.0])
+    thr = sk_synth.digitiser_thresholds(sig).numpy().astype(np.uint32)
+    seed, frame = 0x123456789ABCDEF, 3
+    data = oracle.sim_digitised(T, F, E, thr, seed, frame)
+    for t in range(T):
+        for f in range(F):
+            for e in range(E):
+                w = _philox_py([e // 2, t * F + f, frame & 0xFFFFFFFF, frame >> 32], [seed & 0xFFFFFFFF, seed >> 32])
+                re = -7 + sum(int(w[2 * (e & 1)] >= x) for x in thr[e])
+                im = -7 + sum(int(w[2 * (e & 1) + 1] >= x) for x in thr[e])
+                assert data[t, f, e] == ((re + 8) << 4) | (im + 8)
+    assert not np.array_equal(data, oracle.sim_digitised(T, F, E, thr, seed, frame + 1))
+    # statistics: 2 x 400k components per receiver
+    T = 100000
+    data = oracle.sim_digitised(T, 4, 3, thr[1:4], seed=7)
+    comp = np.stack([(data >> 4).astype(int) - 8, (data & 15).astype(int) - 8])       # [2][T][4][3]
+    assert comp.min() >= -7 and comp.max() <= 7
+    from math import erf, sqrt
+    for i, s_ in enumerate(sig[1:4]):
+        cdf = [0.0] + [0.5 * (1 + erf((j - 6.5) / s_ / sqrt(2))) for j in range(14)] + [1.0]
+        pmf = np.diff(cdf)
+        x = comp[..., i].ravel()
+        n = x.size
+        freq = np.bincount(x + 7, minlength=15) / n
+        assert (np.abs(freq - pmf) < 5 * np.sqrt(pmf * (1 - pmf) / n) + 2e-9).all()
+        rms_model = np.sqrt((pmf * np.arange(-7, 8) ** 2).sum())
+        assert abs(np.sqrt((x.astype(float) ** 2).mean()) - rms_model) < 0.01
+    # the paper's operating point: RMS ~1.52 LSB per component
+    pmf152 = np.diff([0.0] + [0.5 * (1 + erf((j - 6.5) / 1.52 / sqrt(2))) for j in range(14)] + [1.0])
+    assert abs(np.sqrt((pmf152 * np.arange(-7, 8) ** 2).sum()) - 1.52) < 0.04
+
+
+def test_app_b_mean_offset_constant_variance_converges(oracle):
+    """PAPER.md:282-284 on the simulator's data (sigma = 1.52): the mean of SK~ is offset from 1 by
+    a constant that does not depend on N and equals the model's E[p^2]/E[p]^2 - 1; the variance
+    approaches the un-digitised 4/(MN) (here within 15 %)."""
+    import sk_synth
+    M, E, B = 64, 256, 400
+    thr = sk_synth.digitiser_thresholds(np.full(E, 1.52)).numpy().astype(np.uint32)
+    data = oracle.sim_digitised(M * B, 1, E, thr, seed=11)
+    lim = _quantised_limit(1.52)
+    means = {}
+    for N in (16, 64, 256):
+        sk = oracle.frame(data, M, first_n=N)["SK"]
+        mean, var = oracle.moments(sk)
+        means[N] = mean[0]
+        assert abs(mean[0] - lim) < 4 * np.sqrt(4 / (M * N * B)) + 2.0 / M ** 2 + 1e-3
+        assert 0.85 < var[0] / (4 / (M * N)) < 1.15
+    assert abs(means[16] - means[256]) < 5 * np.sqrt(4 / (M * 16 * B))
+
+
+def test_moments(oracle):
+    rng = np.random.default_rng(13)
+    SK = rng.normal(0.94, 0.003, size=(500, 3)).astype(np.float32)
+    mean, var = oracle.moments(SK)
+    np.testing.assert_allclose(mean, SK.astype(np.float64).mean(axis=0), rtol=1e-13)
+    np.testing.assert_allclose(var, SK.astype(np.float64).var(axis=0, ddof=1), rtol=1e-10)
+    assert np.isnan(oracle.moments(SK[:1])[1]).all()
