@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single"],
+    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single", "sim"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
@@ -189,6 +189,44 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sim(args):
+    """--op sim: the App. B simulator (sk_sim_digitised) writing config-1-shaped frames, then the
+    null mean through sk_frame + sk_moments."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    torch.cuda.set_device(0)
+    cfg = sk_synth.config(1)
+    thr = sk_synth.digitiser_thresholds(sk_synth.sigma_per_input(cfg)).cuda()
+    bufs = [torch.empty(cfg.T, cfg.F, cfg.E, dtype=torch.uint8, device="cuda") for _ in range(4)]
+    K, W = args.steps if args.steps != 2000 else 20, max(args.warmup, 3)
+    for i in range(W):
+        sk.sk_sim_digitised(cfg.T, cfg.F, cfg.E, thr, 1, i, out=bufs[i % 4])
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = sk.sk_launch_count()
+    e0.record()
+    for i in range(K):
+        sk.sk_sim_digitised(cfg.T, cfg.F, cfg.E, thr, 1, 100 + i, out=bufs[i % 4])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    mean, var = sk.sk_moments(sk.sk_frame(bufs[0], cfg.M).SK)
+    # issue roofline: the loop body is 225 SASS instructions per row of a receiver pair, i.e. 112 per
+    # sample (Philox4x32-10: 10 rounds x 6; 4 components x 14 compare-adds x 2), one instruction per
+    # cycle per sub-partition: 592 x 32 x 1.965 GHz / 112 = 332 Gsamples/s
+    peak = 592 * 32 * 1.965 / 112
+    print(json.dumps({
+        "op": "sim", "metric": "simulated_samples_per_s", "value": cfg.nbytes / (ms * 1e-3), "unit": "samples/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
+        "dtype": "u32->u8", "config": {"workload": cfg.name + " shape, per-input sigma ~ U[1.5,3.5]",
+                                       "null_mean": float(mean[0].item()), "null_var": float(var[0].item())},
+        "roofline": {"bound": "alu", "achieved": cfg.nbytes / (ms * 1e-3) / 1e9, "unit": "Gsamples/s",
+                     "peak": peak, "frac": cfg.nbytes / (ms * 1e-3) / 1e9 / peak, "traffic": None,
+                     "peak_source": "issue slots: 112 SASS instructions per sample (DESIGN.md section 9)"},
+        "gpu_launches": int(sk.sk_launch_count() - n0) }))
+
+
 def run_aux(args):
     """--op rebin|single: one of the small HBM-bound kernels beside the hot path, on S1/S2 arrays of
     config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), two rotating copies."""
@@ -235,6 +273,8 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.op == "sim":
+        return run_sim(args)
     if args.op != "frame":
         return run_aux(args)
 

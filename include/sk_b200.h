@@ -127,6 +127,22 @@ int sk_single(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, ui
 int sk_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_t N, float sk_mean,
                     float* sig, void* stream);
 
+/* Digitisation simulation (App. B: "4+4-bit complex Gaussian data (bounded
+ * between -7 and 7) with an RMS of ~1.52 least-significant bits in each component").  Fills
+ * data[T][F][E] with seeded samples: for row r = t*F + f and receiver pair j = e/2 the
+ * counter-based generator Philox4x32-10 is called with counter (j, r, frame_lo, frame_hi) and key
+ * (seed_lo, seed_hi); words 0, 1 give (re, im) of receiver 2j, words 2, 3 of receiver 2j+1; a
+ * component is -7 + #{k : word >= thr[e][k]}.  thr: uint32 [E][14] on the device, ascending per
+ * receiver, thr[e][k] = 2^32 * P(component <= k - 7) for the caller's sigma_e.  T*F < 2^32.
+ * Run sk_frame on the result and sk_moments on its SK to get the null mean to pass as sk_mean
+ * ("this offset is added directly to the value of the RFI excision threshold"). */
+int sk_sim_digitised(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, const uint32_t* thr,
+                     uint64_t seed, uint64_t frame, void* stream);
+
+/* Mean and unbiased variance (NaN if B < 2) of SK [B][F] over the blocks, per frequency:
+ * float64 mean[F], var[F] on the device.  Two passes, fixed summation order. */
+int sk_moments(const float* SK, uint32_t B, uint32_t F, double* mean, double* var, void* stream);
+
 /* Text for a return value of the calls above (static storage; never NULL). */
 const char* sk_strerror(int code);
 

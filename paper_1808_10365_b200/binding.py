@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
-           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_strerror", "sk_version",
+           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments",
+           "sk_strerror", "sk_version",
            "sk_launch_count")
 
 _lib = None
@@ -44,12 +45,14 @@ def lib() -> C.CDLL:
     L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
+    L.sk_sim_digitised.argtypes = [vp, u32, u32, u32, vp, C.c_uint64, C.c_uint64, vp]
+    L.sk_moments.argtypes = [vp, u32, u32, vp, vp, vp]
     L.sk_strerror.argtypes = [i32]
     L.sk_strerror.restype = C.c_char_p
     L.sk_version.restype = i32
     L.sk_launch_count.restype = C.c_ulonglong
     for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host", "sk_rebin_sums",
-                 "sk_single", "sk_significance"):
+                 "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments"):
         getattr(L, name).restype = i32
     _lib = L
     return L
@@ -195,6 +198,30 @@ def sk_significance(SK: torch.Tensor, M: int, N: int, sk_mean: float = 1.0, stre
     _check(lib().sk_significance(SK.data_ptr(), B, F, M, N, sk_mean, sig.data_ptr(), _stream(stream)),
            "sk_significance")
     return sig
+
+
+def sk_sim_digitised(T: int, F: int, E: int, thr: torch.Tensor, seed: int, frame: int = 0, out=None, stream=None):
+    """PAPER.md:276-284 (App. B): seeded 4+4-bit round-and-clip Gaussian frame uint8 [T][F][E] on
+    thr's device; thr uint32 [E][14] (sk_synth.digitiser_thresholds)."""
+    _dev(thr, torch.uint32, "thr")
+    if tuple(thr.shape) != (E, 14):
+        raise SKError("thr must be [E][14]")
+    if out is None:
+        out = torch.empty((T, F, E), dtype=torch.uint8, device=thr.device)
+    _dev(out, torch.uint8, "out")
+    _check(lib().sk_sim_digitised(out.data_ptr(), T, F, E, thr.data_ptr(), seed, frame, _stream(stream)),
+           "sk_sim_digitised")
+    return out
+
+
+def sk_moments(SK: torch.Tensor, stream=None):
+    """Mean and unbiased variance of SK float32 [B][F] over the blocks: float64 [F] each."""
+    _dev(SK, torch.float32, "SK")
+    B, F = SK.shape
+    mean = torch.empty(F, dtype=torch.float64, device=SK.device)
+    var = torch.empty(F, dtype=torch.float64, device=SK.device)
+    _check(lib().sk_moments(SK.data_ptr(), B, F, mean.data_ptr(), var.data_ptr(), _stream(stream)), "sk_moments")
+    return mean, var
 
 
 def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: float = 3.0,

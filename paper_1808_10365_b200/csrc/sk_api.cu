@@ -9,6 +9,7 @@
 #include "../../include/sk_b200.h"
 #include "sk_kernels.cuh"
 #include "sk_tma.cuh"
+#include "sk_sim.cuh"
 
 #include <cstdlib>
 #include <cstring>
@@ -400,6 +401,30 @@ int sk_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_
     const double sd = std::sqrt(4.0 / ((double)M * (double)N));
     sk::sk_significance_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
         SK, sig, cells, (double)sk_mean, sd);
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_sim_digitised(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, const uint32_t* thr, uint64_t seed,
+                     uint64_t frame, void* stream) {
+    if (!data || !thr) return SK_ERR_NULL;
+    if (T == 0 || F == 0 || E == 0 || (unsigned long long)T * F > 0xFFFFFFFFull) return SK_ERR_SHAPE;
+    const unsigned long long rows = (unsigned long long)T * F;
+    unsigned long long rpt = (rows + 65534ull) / 65535ull;          // rows per thread: grid.y <= 65535
+    if (rpt < (unsigned long long)sk::kSimRows) rpt = sk::kSimRows;
+    const uint32_t pairs = (E + 1) / 2;
+    const dim3 grid((pairs + sk::kSimThreads - 1) / sk::kSimThreads, (unsigned)((rows + rpt - 1) / rpt));
+    sk::sk_sim_kernel<<<grid, sk::kSimThreads, 0, (cudaStream_t)stream>>>(
+        data, rows, (uint32_t)rpt, E, thr, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)frame,
+        (uint32_t)(frame >> 32));
+    ++g_launches;
+    return launch_status();
+}
+
+int sk_moments(const float* SK, uint32_t B, uint32_t F, double* mean, double* var, void* stream) {
+    if (!SK || !mean || !var) return SK_ERR_NULL;
+    if (B == 0 || F == 0) return SK_ERR_SHAPE;
+    sk::sk_moments_kernel<<<F, sk::kMomThreads, 0, (cudaStream_t)stream>>>(SK, B, F, mean, var);
     ++g_launches;
     return launch_status();
 }

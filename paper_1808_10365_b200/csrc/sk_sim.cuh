@@ -1,0 +1,106 @@
+// sk_sim.cuh — SURVEY.md section 8(f) NEXT-1: the digitisation simulation of PAPER.md:276-284
+// (App. B) on the device: seeded 4+4-bit round-and-clip Gaussian frames generated straight into
+// HBM, and the mean / variance of the SK estimates.  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace sk {
+
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): counter-based, so every (row, receiver pair)
+// draws its four words independently of the launch shape.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0;
+        c1 = l1;
+        c2 = h0 ^ c3 ^ k1;
+        c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// value + 8 = 1 + #{ j : u >= thr[j] }  (value = -7 + count): thresholds in registers, no branches.
+__device__ __forceinline__ uint32_t digitise_nibble(uint32_t u, const uint32_t (&thr)[14]) {
+    uint32_t n = 1;
+#pragma unroll
+    for (int j = 0; j < 14; ++j) n += (u >= thr[j]) ? 1u : 0u;
+    return n;
+}
+
+constexpr int kSimThreads = 128;
+constexpr int kSimRows = 64;              // rows per thread (at least)
+
+// Thread = one receiver pair (2j, 2j+1) for rpt rows r = t*F + f; counter (j, r, frame), key seed.
+__global__ void __launch_bounds__(kSimThreads)
+sk_sim_kernel(uint8_t* __restrict__ data, uint64_t rows, uint32_t rpt, uint32_t E, const uint32_t* __restrict__ thr,
+              uint32_t seed_lo, uint32_t seed_hi, uint32_t frame_lo, uint32_t frame_hi) {
+    const uint32_t j = blockIdx.x * kSimThreads + threadIdx.x;
+    const uint32_t e = 2 * j;
+    if (e >= E) return;
+    const bool two = e + 1 < E;
+    uint32_t ta[14], tb[14];
+#pragma unroll
+    for (int i = 0; i < 14; ++i) {
+        ta[i] = __ldg(thr + (size_t)e * 14 + i);
+        tb[i] = two ? __ldg(thr + (size_t)(e + 1) * 14 + i) : 0u;
+    }
+    const uint64_t r0 = (uint64_t)blockIdx.y * rpt;
+    const uint64_t r1 = r0 + rpt < rows ? r0 + rpt : rows;
+    for (uint64_t r = r0; r < r1; ++r) {
+        uint32_t w[4];
+        philox4x32_10(j, (uint32_t)r, frame_lo, frame_hi, seed_lo, seed_hi, w);
+        const uint32_t a = (digitise_nibble(w[0], ta) << 4) | digitise_nibble(w[1], ta);
+        uint8_t* q = data + r * E + e;
+        if (two) {
+            const uint32_t b = (digitise_nibble(w[2], tb) << 4) | digitise_nibble(w[3], tb);
+            if ((reinterpret_cast<uintptr_t>(q) & 1u) == 0) *reinterpret_cast<uint16_t*>(q) = (uint16_t)(a | (b << 8));
+            else { q[0] = (uint8_t)a; q[1] = (uint8_t)b; }
+        } else {
+            q[0] = (uint8_t)a;
+        }
+    }
+}
+
+// Mean and unbiased variance of SK over the blocks, per frequency: one CTA per frequency, two
+// passes in float64, fixed order (thread-strided partial sums, then a shared-memory tree).
+constexpr int kMomThreads = 256;
+
+__device__ __forceinline__ double block_sum(double x, double* red) {
+    red[threadIdx.x] = x;
+    __syncthreads();
+    for (int o = kMomThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] = __dadd_rn(red[threadIdx.x], red[threadIdx.x + o]);
+        __syncthreads();
+    }
+    const double s = red[0];
+    __syncthreads();
+    return s;
+}
+
+__global__ void __launch_bounds__(kMomThreads)
+sk_moments_kernel(const float* __restrict__ SK, uint32_t B, uint32_t F, double* __restrict__ mean,
+                  double* __restrict__ var) {
+    __shared__ double red[kMomThreads];
+    const uint32_t f = blockIdx.x;
+    double s = 0.0;
+    for (uint32_t b = threadIdx.x; b < B; b += kMomThreads) s = __dadd_rn(s, (double)SK[(size_t)b * F + f]);
+    const double m = __ddiv_rn(block_sum(s, red), (double)B);
+    double v = 0.0;
+    for (uint32_t b = threadIdx.x; b < B; b += kMomThreads) {
+        const double d = __dsub_rn((double)SK[(size_t)b * F + f], m);
+        v = __fma_rn(d, d, v);
+    }
+    v = block_sum(v, red);
+    if (threadIdx.x == 0) {
+        mean[f] = m;
+        var[f] = B > 1 ? __ddiv_rn(v, (double)(B - 1)) : __longlong_as_double(0x7ff8000000000000ll);
+    }
+}
+
+}  // namespace sk

@@ -421,6 +421,41 @@ def test_constant_modulus_is_exactly_zero_on_device(sk):
         assert bool((sk.sk_single(out.S1, out.S2, M) == 0).all())
 
 
+@pytest.mark.parametrize("T,F,E", [(70, 3, 37), (256, 1, 2048), (129, 2, 258), (1, 1, 1)])
+def test_sim_digitised_bytes_bit_exact(sk, oracle, T, F, E):
+    """the device's digitisation simulator and the oracle's
+    produce the same bytes from the same thresholds, seed and frame (odd E, ragged row chunks)."""
+    rng = np.random.default_rng(E)
+    sig = rng.uniform(0.5, 4.0, size=E)
+    thr = sk_synth.digitiser_thresholds(sig)
+    for seed, frame in ((1, 0), (0xFEDCBA9876543210, 5)):
+        got = sk.sk_sim_digitised(T, F, E, thr.cuda(), seed, frame)
+        ref = oracle.sim_digitised(T, F, E, thr.numpy().astype(np.uint32), seed, frame)
+        np.testing.assert_array_equal(got.cpu().numpy(), ref)
+
+
+def test_sim_null_mean_feeds_the_flag(sk, oracle):
+    """The App. B loop end to end on the device: simulate an RFI-free frame with config 1's
+    per-input sigmas, take the null mean and variance of SK (sk_moments against the oracle), and
+    flag a real config-1 frame with it: nothing is flagged at 5 sigma, whereas the literal centre
+    1.0 flags everything."""
+    cfg = sk_synth.config(1)
+    sig = sk_synth.sigma_per_input(cfg)
+    thr = sk_synth.digitiser_thresholds(sig).cuda()
+    sim = sk.sk_sim_digitised(64 * cfg.M, 1, cfg.E, thr, seed=2018, frame=0)
+    out = sk.sk_frame(sim, cfg.M)
+    mean, var = sk.sk_moments(out.SK)
+    rmean, rvar = oracle.moments(out.SK.cpu().numpy())
+    np.testing.assert_allclose(mean.cpu().numpy(), rmean, rtol=1e-12)
+    np.testing.assert_allclose(var.cpu().numpy(), rvar, rtol=1e-9)
+    null_mean = float(mean[0].item())
+    assert 0.90 < null_mean < 0.93
+    assert float(var[0].item()) < 4.0 / (cfg.M * cfg.E)             # below first order on 4-bit data
+    frame = sk_synth.make_frame(cfg.with_(T=32 * cfg.M), device="cuda")
+    assert int(sk.sk_frame(frame, cfg.M, n_sigma=5.0, sk_mean=null_mean).mask.sum().item()) == 0
+    assert bool(sk.sk_frame(frame, cfg.M, n_sigma=5.0, sk_mean=1.0).mask.all())
+
+
 def test_empty_subset_is_nan_and_flagged(sk):
     data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
     out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
