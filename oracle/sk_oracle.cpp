@@ -344,6 +344,67 @@ int sk_oracle_moments(const float* SK, uint32_t B, uint32_t F, double* mean, dou
     return 0;
 }
 
-int sk_oracle_version(void) { return 3; }
+// ---------------------------------------------------------------------------------------------
+// the common-mode simulation of PAPER.md:262-272 (App. A, Fig. 5).
+// "a number of independent Gaussian datasets, representing the noise-dominated receiver
+// timestreams, are augmented by a common-mode Gaussian signal representing the 'source'."
+//
+// One complex circular Gaussian (unit variance per component) from two 32-bit words: Box-Muller,
+// u1 = (w0 + 0.5) / 2^32 in (0, 1), u2 = (w1 + 0.5) / 2^32:
+//   z = sqrt(-2 ln u1) * (cos 2 pi u2, sin 2 pi u2).
+static inline void gauss_pair(uint32_t w0, uint32_t w1, double& re, double& im) {
+    const double u1 = ((double)w0 + 0.5) / 4294967296.0, u2 = ((double)w1 + 0.5) / 4294967296.0;
+    const double rad = std::sqrt(-2.0 * std::log(u1)), ang = 6.283185307179586476925286766559 * u2;
+    re = rad * std::cos(ang);
+    im = rad * std::sin(ang);
+}
+
+int sk_oracle_gauss_pair(uint32_t w0, uint32_t w1, double* out) {
+    if (!out) return -1;
+    gauss_pair(w0, w1, out[0], out[1]);
+    return 0;
+}
+
+// Sample (dataset d, time t, receiver e): x = z + amp * c, with
+//   z from Philox counter (e/2, t, d, 0), words 0,1 (even e) or 2,3 (odd e),
+//   c from Philox counter (0,   t, d, 1), words 0,1 (the same for all receivers),
+// key (seed_lo, seed_hi).  x_out (optional): [D][M][N][2] doubles, for tests.
+// SK64[d] = Eq. 14 over the N receivers and the M samples of dataset d (float64 sums, Eq. 7, 9-11).
+int sk_oracle_sim_common_mode(uint32_t D, uint32_t M, uint32_t N, double amp, uint64_t seed,
+                              double* SK64, double* x_out) {
+    if (!SK64 || D == 0 || M < 2 || N == 0) return -1;
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    const double n = (double)M;
+    for (uint32_t d = 0; d < D; ++d) {
+        double S2bar = 0.0;
+        for (uint32_t e = 0; e < N; ++e) {
+            double s1 = 0.0, s2 = 0.0;
+            for (uint32_t t = 0; t < M; ++t) {
+                const uint32_t cz[4] = {e / 2, t, d, 0u}, cc[4] = {0u, t, d, 1u};
+                uint32_t wz[4], wc[4];
+                philox4x32_10(cz, key, wz);
+                philox4x32_10(cc, key, wc);
+                double zr, zi, cr, ci;
+                gauss_pair(wz[2 * (e & 1)], wz[2 * (e & 1) + 1], zr, zi);
+                gauss_pair(wc[0], wc[1], cr, ci);
+                const double xr = zr + amp * cr, xi = zi + amp * ci;
+                if (x_out) {
+                    const size_t i = (((size_t)d * M + t) * N + e) * 2;
+                    x_out[i] = xr;
+                    x_out[i + 1] = xi;
+                }
+                const double p = xr * xr + xi * xi;       // Eq. 7
+                s1 += p;
+                s2 += p * p;
+            }
+            const double mu = s1 / n;                      // Eq. 9
+            S2bar += (s1 == 0.0) ? n : s2 / (mu * mu);     // Eq. 11
+        }
+        SK64[d] = (n + 1.0) / (n - 1.0) * (S2bar / (n * (double)N) - 1.0);   // Eq. 14
+    }
+    return 0;
+}
+
+int sk_oracle_version(void) { return 4; }
 
 }  // extern "C"

@@ -209,3 +209,21 @@ def moments(SK):
     _check(lib().sk_oracle_moments(_p(SK, C.c_float), B, F, _p(mean, C.c_double), _p(var, C.c_double)),
            "sk_oracle_moments")
     return mean, var
+
+
+def gauss_pair(w0, w1):
+    """Box-Muller: two 32-bit words -> one circular complex Gaussian (re, im), unit variance each."""
+    out = np.empty(2, dtype=np.float64)
+    _check(lib().sk_oracle_gauss_pair(C.c_uint32(int(w0)), C.c_uint32(int(w1)), _p(out, C.c_double)), "gauss_pair")
+    return out
+
+
+def sim_common_mode(D, M, N, amp, seed, want_x=False):
+    """PAPER.md:262-272 (App. A): D datasets of M samples x N receivers of unit Gaussian noise plus
+    amp x a common-mode Gaussian; returns SK~ per dataset (float64 [D]) and optionally the samples
+    complex128 [D][M][N]."""
+    SK = np.empty(D, dtype=np.float64)
+    x = np.empty((D, M, N, 2), dtype=np.float64) if want_x else None
+    _check(lib().sk_oracle_sim_common_mode(D, M, N, C.c_double(amp), C.c_uint64(seed), _p(SK, C.c_double),
+                                           _p(x, C.c_double)), "sk_oracle_sim_common_mode")
+    return (SK, x[..., 0] + 1j * x[..., 1]) if want_x else SK

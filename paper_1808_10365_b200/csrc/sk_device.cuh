@@ -173,6 +173,10 @@ struct AccSplit {
         add_c<I, 3>(pick<3>(r, m));
     }
     __device__ __forceinline__ void add16(const uint4& v, const UnpackConsts& kc) {
+#ifdef SK_PROBE_MEMORY_ONLY                         // experiments only: what the load path alone sustains
+        b[0].r += v.x ^ v.y ^ v.z ^ v.w;
+        return;
+#endif
         add_word<0>(v.x, kc);
         add_word<1>(v.y, kc);
         add_word<2>(v.z, kc);

@@ -492,3 +492,55 @@ def test_moments(oracle):
     np.testing.assert_allclose(mean, SK.astype(np.float64).mean(axis=0), rtol=1e-13)
     np.testing.assert_allclose(var, SK.astype(np.float64).var(axis=0, ddof=1), rtol=1e-10)
     assert np.isnan(oracle.moments(SK[:1])[1]).all()
+
+
+# ---- App. A common-mode simulation ----------------------
+def test_gauss_pair_and_common_mode_samples(oracle):
+    """Box-Muller against its definition at chosen words, then the simulated samples: unit variance
+    per component, E|z|^4 = 8 (circular Gaussian, variance 2), independent receivers when amp = 0,
+    correlation amp^2/(1+amp^2) between receivers otherwise, and the counter layout (receiver pairs
+    share one Philox call; the common-mode term is the same for every receiver)."""
+    z = oracle.gauss_pair(0x7FFFFFFF, 0)                        # u1 = 0.5 - 2^-33 + ..., u2 = 2^-33
+    assert z[0] == pytest.approx(math.sqrt(-2 * math.log((0x7FFFFFFF + 0.5) / 2 ** 32)) * math.cos(2 * math.pi * 0.5 / 2 ** 32), rel=1e-14)
+    assert abs(z[1]) < 1e-8
+    z = oracle.gauss_pair(0, 0x40000000)                        # u2 ~ 1/4: on the imaginary axis
+    assert abs(z[0]) < 1e-7 and z[1] == pytest.approx(math.sqrt(-2 * math.log(0.5 / 2 ** 32)), rel=1e-9)
+    D, M, N = 40, 64, 16
+    sk0, x0 = oracle.sim_common_mode(D, M, N, 0.0, seed=5, want_x=True)
+    sk1, x1 = oracle.sim_common_mode(D, M, N, 1.5, seed=5, want_x=True)
+    n = x0.size
+    assert abs(x0.real.var() - 1) < 5 * math.sqrt(2 / n) and abs(x0.imag.var() - 1) < 5 * math.sqrt(2 / n)
+    assert abs((np.abs(x0) ** 4).mean() - 8) < 5 * math.sqrt((384 - 64) / n)
+    assert abs(x0.mean()) < 5 * math.sqrt(2 / n)
+    c = (x1 - x0) / 1.5                                           # the common-mode term
+    assert np.allclose(c, c[:, :, :1], atol=1e-12) and abs(c[:, :, 0].real.var() - 1) < 0.1
+    a = x0.reshape(-1, N)
+    corr0 = (a[:, 0] * np.conj(a[:, 1])).mean() / 2
+    assert abs(corr0) < 5 / math.sqrt(a.shape[0])
+    b = x1.reshape(-1, N)
+    corr1 = ((b[:, 0] * np.conj(b[:, 1])).mean() / (np.abs(b[:, 0]) ** 2).mean()).real
+    assert corr1 == pytest.approx(1.5 ** 2 / (1 + 1.5 ** 2), abs=0.06)
+    # Eq. 14 of these samples, recomputed with numpy from the returned x
+    p = np.abs(x1) ** 2
+    S1, S2 = p.sum(axis=1), (p ** 2).sum(axis=1)
+    want = (M + 1) / (M - 1) * ((M * M * S2 / S1 ** 2).sum(axis=1) / (M * N) - 1)
+    np.testing.assert_allclose(sk1, want, rtol=1e-12)
+
+
+def test_app_a_effective_receivers(oracle):
+    """PAPER.md:266-272 (Fig. 5): with no common mode var(SK~) = 4/(nN) (N_eff = N); as the
+    common-mode amplitude grows the variance rises towards the single-receiver value (N_eff -> 1);
+    a larger array loses a larger share of its receivers at the same amplitude."""
+    M, D = 64, 600
+    exact = lambda N: 4.0 * M * M / ((M - 1) * (M + 2) * (M + 3) * N)      # Gaussian value of 4/(nN)
+    neff = {}
+    for N in (8, 64):
+        for amp in (0.0, 0.5, 4.0):
+            sk = oracle.sim_common_mode(D, M, N, amp, seed=17 + N)
+            neff[N, amp] = exact(1) / sk.var(ddof=1)
+            assert abs(sk.mean() - 1) < 5 * math.sqrt(exact(1) / D)
+    for N in (8, 64):
+        assert neff[N, 0.0] == pytest.approx(N, rel=0.25)
+        assert neff[N, 0.0] > neff[N, 0.5] > neff[N, 4.0]
+        assert neff[N, 4.0] < 1.6                                   # effectively a single receiver
+    assert neff[64, 0.5] / 64 < neff[8, 0.5] / 8                    # larger arrays suffer first
