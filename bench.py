@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single", "sim"],
+    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single", "sim", "cm"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
@@ -227,6 +227,34 @@ def run_sim(args):
         "gpu_launches": int(sk.sk_launch_count() - n0) }))
 
 
+def run_cm(args):
+    """--op cm: one point of Fig. 5: 1000 datasets, n = 256, N = 4096 receivers."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    torch.cuda.set_device(0)
+    D, M, N, amp = 1000, 256, 4096, 0.5
+    K, W = args.steps if args.steps != 2000 else 5, 3
+    for i in range(W):
+        sk.sk_sim_common_mode(D, M, N, amp, seed=i)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = sk.sk_launch_count()
+    e0.record()
+    for i in range(K):
+        SK = sk.sk_sim_common_mode(D, M, N, amp, seed=100 + i)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    mean, var = sk.sk_moments(SK)
+    print(json.dumps({
+        "op": "cm", "metric": "simulated_samples_per_s", "value": D * M * N / (ms * 1e-3), "unit": "samples/s",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
+        "dtype": "f64", "config": {"workload": f"App. A: {D} datasets x n={M} x N={N}, common-mode amplitude {amp}",
+                                   "mean": float(mean[0].item()), "var": float(var[0].item()),
+                                   "n_eff": 4.0 / (M * float(var[0].item()))},
+        "roofline": None, "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
 def run_aux(args):
     """--op rebin|single: one of the small HBM-bound kernels beside the hot path, on S1/S2 arrays of
     config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), two rotating copies."""
@@ -275,6 +303,8 @@ def main():
         return run_reference(args)
     if args.op == "sim":
         return run_sim(args)
+    if args.op == "cm":
+        return run_cm(args)
     if args.op != "frame":
         return run_aux(args)
 

@@ -139,6 +139,16 @@ int sk_significance(const float* SK, uint32_t B, uint32_t F, uint32_t M, uint32_
 int sk_sim_digitised(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, const uint32_t* thr,
                      uint64_t seed, uint64_t frame, void* stream);
 
+/* Common-mode simulation (App. A, Fig. 5): D independent datasets of M time
+ * samples x N receivers, x = z + amp * c with z independent unit circular complex Gaussians and c
+ * one common circular Gaussian per time sample; writes SK[d] = Eq. 14 of dataset d (float64
+ * inside, float32 out; the samples are never stored).  Random numbers: Philox4x32-10, key
+ * (seed_lo, seed_hi), counter (e/2, t, d, 0) for the receivers (words 0,1 / 2,3 = receivers 2j /
+ * 2j+1) and (0, t, d, 1) for c; a Gaussian pair is the Box-Muller transform of two words.
+ * 2 <= M <= 2048.  sk_moments(SK, D, 1) then gives var(SK) and N_eff = 4 / (M var). */
+int sk_sim_common_mode(uint32_t D, uint32_t M, uint32_t N, double amp, uint64_t seed, float* SK,
+                       void* stream);
+
 /* Mean and unbiased variance (NaN if B < 2) of SK [B][F] over the blocks, per frequency:
  * float64 mean[F], var[F] on the device.  Two passes, fixed summation order. */
 int sk_moments(const float* SK, uint32_t B, uint32_t F, double* mean, double* var, void* stream);

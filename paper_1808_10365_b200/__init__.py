@@ -5,9 +5,9 @@ its thin Python binding.  See DESIGN.md.
 """
 from .binding import (SKError, SKResult, LIB_PATH, SYMBOLS, lib, sk_combine, sk_flag, sk_frame,
                       sk_frame_host, sk_frame_workspace_bytes, sk_launch_count, sk_power_sums,
-                      sk_moments, sk_rebin_sums, sk_significance, sk_sim_digitised, sk_single, sk_strerror, sk_version, workspace_for)
+                      sk_moments, sk_rebin_sums, sk_significance, sk_sim_common_mode, sk_sim_digitised, sk_single, sk_strerror, sk_version, workspace_for)
 
 __all__ = ["SKError", "SKResult", "LIB_PATH", "SYMBOLS", "lib", "sk_combine", "sk_flag", "sk_frame",
            "sk_frame_host", "sk_frame_workspace_bytes", "sk_launch_count", "sk_power_sums",
-           "sk_moments", "sk_rebin_sums", "sk_significance", "sk_sim_digitised", "sk_single",
+           "sk_moments", "sk_rebin_sums", "sk_significance", "sk_sim_common_mode", "sk_sim_digitised", "sk_single",
            "sk_strerror", "sk_version", "workspace_for"]

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
-           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments",
+           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments",
            "sk_strerror", "sk_version",
            "sk_launch_count")
 
@@ -47,12 +47,13 @@ def lib() -> C.CDLL:
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
     L.sk_sim_digitised.argtypes = [vp, u32, u32, u32, vp, C.c_uint64, C.c_uint64, vp]
     L.sk_moments.argtypes = [vp, u32, u32, vp, vp, vp]
+    L.sk_sim_common_mode.argtypes = [u32, u32, u32, C.c_double, C.c_uint64, vp, vp]
     L.sk_strerror.argtypes = [i32]
     L.sk_strerror.restype = C.c_char_p
     L.sk_version.restype = i32
     L.sk_launch_count.restype = C.c_ulonglong
     for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host", "sk_rebin_sums",
-                 "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments"):
+                 "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments", "sk_sim_common_mode"):
         getattr(L, name).restype = i32
     _lib = L
     return L
@@ -212,6 +213,16 @@ def sk_sim_digitised(T: int, F: int, E: int, thr: torch.Tensor, seed: int, frame
     _check(lib().sk_sim_digitised(out.data_ptr(), T, F, E, thr.data_ptr(), seed, frame, _stream(stream)),
            "sk_sim_digitised")
     return out
+
+
+def sk_sim_common_mode(D: int, M: int, N: int, amp: float, seed: int, device="cuda", stream=None):
+    """PAPER.md:262-272 (App. A): SK~ of D simulated datasets (M samples x N receivers, common-mode
+    amplitude amp): float32 [D][1] on `device` (shape ready for sk_moments)."""
+    SK = torch.empty((D, 1), dtype=torch.float32, device=device)
+    if not SK.is_cuda:
+        raise SKError("sk_sim_common_mode needs a CUDA device (there is no CPU fallback)")
+    _check(lib().sk_sim_common_mode(D, M, N, float(amp), seed, SK.data_ptr(), _stream(stream)), "sk_sim_common_mode")
+    return SK
 
 
 def sk_moments(SK: torch.Tensor, stream=None):

@@ -421,6 +421,18 @@ int sk_sim_digitised(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, const ui
     return launch_status();
 }
 
+int sk_sim_common_mode(uint32_t D, uint32_t M, uint32_t N, double amp, uint64_t seed, float* SK, void* stream) {
+    if (!SK) return SK_ERR_NULL;
+    if (M < 2 || M > 2048) return SK_ERR_M;             // the common-mode samples live in shared memory
+    if (D == 0 || D > 0x7fffffffu) return SK_ERR_SHAPE;
+    if (N == 0) return SK_ERR_N;
+    if (!std::isfinite(amp)) return SK_ERR_PARAM;
+    sk::sk_sim_common_mode_kernel<<<D, sk::kCmThreads, (size_t)M * sizeof(double2), (cudaStream_t)stream>>>(
+        M, N, amp, (uint32_t)seed, (uint32_t)(seed >> 32), SK);
+    ++g_launches;
+    return launch_status();
+}
+
 int sk_moments(const float* SK, uint32_t B, uint32_t F, double* mean, double* var, void* stream) {
     if (!SK || !mean || !var) return SK_ERR_NULL;
     if (B == 0 || F == 0) return SK_ERR_SHAPE;

@@ -5,6 +5,8 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "sk_kernels.cuh"
+
 namespace sk {
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): counter-based, so every (row, receiver pair)
@@ -101,6 +103,76 @@ sk_moments_kernel(const float* __restrict__ SK, uint32_t B, uint32_t F, double* 
         mean[f] = m;
         var[f] = B > 1 ? __ddiv_rn(v, (double)(B - 1)) : __longlong_as_double(0x7ff8000000000000ll);
     }
+}
+
+// ------------------------------------------------------------------ SURVEY 8(f) NEXT-3 (App. A)
+// Common-mode simulation (Fig. 5): dataset d holds M samples of N receivers,
+// x = z + amp * c, z independent unit circular Gaussians, c one common circular Gaussian per time
+// sample.  One CTA per dataset; the samples never touch HBM: Philox words -> Box-Muller -> float64
+// sums S1, S2 per receiver (Eq. 7) -> Eq. 11 terms -> canonical tree -> Eq. 14.
+__device__ __forceinline__ void gauss_pair(uint32_t w0, uint32_t w1, double& re, double& im) {
+    const double u1 = ((double)w0 + 0.5) * (1.0 / 4294967296.0), u2 = ((double)w1 + 0.5) * (1.0 / 4294967296.0);
+    const double rad = sqrt(-2.0 * log(u1));
+    double sn, cs;
+    sincos(6.283185307179586476925286766559 * u2, &sn, &cs);
+    re = rad * cs;
+    im = rad * sn;
+}
+
+constexpr int kCmThreads = 256;
+
+__global__ void __launch_bounds__(kCmThreads)
+sk_sim_common_mode_kernel(uint32_t M, uint32_t N, double amp, uint32_t seed_lo, uint32_t seed_hi,
+                          float* __restrict__ SK) {
+    extern __shared__ double2 cm[];                 // amp * c(t), t < M
+    __shared__ double red[kCmThreads];
+    const uint32_t d = blockIdx.x;
+    for (uint32_t t = threadIdx.x; t < M; t += kCmThreads) {
+        uint32_t w[4];
+        philox4x32_10(0u, t, d, 1u, seed_lo, seed_hi, w);
+        double cr, ci;
+        gauss_pair(w[0], w[1], cr, ci);
+        cm[t] = make_double2(amp * cr, amp * ci);
+    }
+    __syncthreads();
+    const double Md = (double)M, MM = Md * Md;
+    TreeMerge tm;
+    for (uint32_t e0 = 0; e0 < N; e0 += 2 * kCmThreads) {          // 512 receivers per pass
+        const uint32_t j = e0 / 2 + threadIdx.x, e = 2 * j;
+        double term = 0.0;
+        if (e < N) {
+            double a1 = 0.0, a2 = 0.0, b1 = 0.0, b2 = 0.0;
+            for (uint32_t t = 0; t < M; ++t) {
+                uint32_t w[4];
+                philox4x32_10(j, t, d, 0u, seed_lo, seed_hi, w);
+                double zr, zi;
+                gauss_pair(w[0], w[1], zr, zi);
+                const double2 c = cm[t];
+                double xr = zr + c.x, xi = zi + c.y;
+                double pw = xr * xr + xi * xi;
+                a1 += pw;
+                a2 += pw * pw;
+                gauss_pair(w[2], w[3], zr, zi);
+                xr = zr + c.x;
+                xi = zi + c.y;
+                pw = xr * xr + xi * xi;
+                b1 += pw;
+                b2 += pw * pw;
+            }
+            term = a1 == 0.0 ? Md : MM * a2 / (a1 * a1);
+            if (e + 1 < N) term += (b1 == 0.0 ? Md : MM * b2 / (b1 * b1));
+        }
+        red[threadIdx.x] = term;
+        __syncthreads();
+        for (int o = 1; o < kCmThreads; o <<= 1) {
+            if ((threadIdx.x & (2 * o - 1)) == 0) red[threadIdx.x] += red[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) tm.push(red[0]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0)
+        SK[d] = (float)((Md + 1.0) / (Md - 1.0) * (tm.total() / (Md * (double)N) - 1.0));
 }
 
 }  // namespace sk

@@ -456,6 +456,34 @@ def test_sim_null_mean_feeds_the_flag(sk, oracle):
     assert bool(sk.sk_frame(frame, cfg.M, n_sigma=5.0, sk_mean=1.0).mask.all())
 
 
+@pytest.mark.parametrize("D,M,N,amp", [(12, 64, 16, 0.0), (9, 33, 7, 1.5), (5, 256, 1030, 0.3), (3, 2, 1, 2.0)])
+def test_sim_common_mode_matches_oracle(sk, oracle, D, M, N, amp):
+    """SK~ of every simulated dataset against the oracle's
+    (same Philox counters, Box-Muller in float64 on both sides; odd N, several 512-receiver passes)."""
+    got = sk.sk_sim_common_mode(D, M, N, amp, seed=99).cpu().numpy()[:, 0]
+    ref = oracle.sim_common_mode(D, M, N, amp, seed=99)
+    assert_sk_close(got, ref)
+    assert not np.array_equal(got, sk.sk_sim_common_mode(D, M, N, amp, seed=100).cpu().numpy()[:, 0])
+
+
+def test_sim_common_mode_effective_receivers(sk):
+    """Fig. 5 on the device at the paper's scale (n = 256, 1000 datasets per point): N_eff = N
+    without a common mode, falling towards 1 as it grows, larger arrays first."""
+    M, D = 256, 1000
+    exact1 = 4.0 * M * M / ((M - 1) * (M + 2) * (M + 3))
+    neff = {}
+    for N in (128, 1024):
+        for amp in (0.0, 0.5, 1.0, 3.0):       # receiver correlation rho = amp^2/(1+amp^2); SK_i's ~ rho^4
+            mean, var = sk.sk_moments(sk.sk_sim_common_mode(D, M, N, amp, seed=N))
+            assert abs(mean.item() - 1) < 5 * (exact1 / D) ** 0.5
+            neff[N, amp] = exact1 / var.item()
+    for N in (128, 1024):
+        assert abs(neff[N, 0.0] / N - 1) < 0.2
+        assert neff[N, 0.0] > neff[N, 0.5] > neff[N, 1.0] > neff[N, 3.0]
+        assert neff[N, 3.0] < 1.6
+    assert neff[1024, 0.5] / 1024 < 0.8 * neff[128, 0.5] / 128
+
+
 def test_empty_subset_is_nan_and_flagged(sk):
     data = sk_synth.random_bytes(64, 1, 32, seed=1).cuda()
     out = sk.sk_frame(data, 32, subset=np.zeros(32, bool))
