@@ -61,6 +61,9 @@ SHAPES = [
     (8, 1, 16, 2), (21, 2, 16, 7), (128, 3, 48, 64), (500, 1, 256, 250), (512, 2, 272, 256),
     (768, 1, 2048, 256), (512, 3, 2064, 128), (2048, 1, 512, 1024), (2000, 2, 96, 1000),
     (1024, 5, 32, 512), (66, 1, 4096, 33),
+    # beyond the stream kernel: more than 65535 blocks (grid.z), and blocks too long for its
+    # accumulators (direct-load kernel with AccWide, then AccPlain)
+    (140000, 1, 16, 2), (16384, 1, 32, 8192), (65536, 1, 48, 32768),
 ]
 
 
