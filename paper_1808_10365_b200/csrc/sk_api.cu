@@ -194,7 +194,8 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
         if (tma_wanted(pl)) {
             const int rc = launch_stream(pl.L, p, st);
             if (rc != SK_OK) return rc;
-        } else if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
+        } else if (pl.stream) launch_vec_L<sk::AccChain>(pl.L, p, st);
+        else if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
         else                launch_vec_L<sk::AccPlain>(pl.L, p, st);
     } else {
         sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);

@@ -79,6 +79,7 @@ struct AccPlain {
     static constexpr uint32_t kAddend = 0u;
     __device__ __forceinline__ void reset() { s1 = 0; s2 = 0; }
     __device__ __forceinline__ void add(uint32_t q) { const uint32_t p = q >> 9; s1 += p; s2 += p * p; }
+    __device__ __forceinline__ void add_c(uint32_t c) { add((uint32_t)__dp4a((int)c, (int)c, 0)); }
     __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const { S1 = s1; S2 = s2; }
 };
 
@@ -136,10 +137,10 @@ __device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v, con
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
-        acc[4 * i + 0].add(power512<0>(r, m, Acc::kAddend));
-        acc[4 * i + 1].add(power512<1>(r, m, Acc::kAddend));
-        acc[4 * i + 2].add(power512<2>(r, m, Acc::kAddend));
-        acc[4 * i + 3].add(power512<3>(r, m, Acc::kAddend));
+        acc[4 * i + 0].add_c(pick<0>(r, m));
+        acc[4 * i + 1].add_c(pick<1>(r, m));
+        acc[4 * i + 2].add_c(pick<2>(r, m));
+        acc[4 * i + 3].add_c(pick<3>(r, m));
     }
 }
 
