@@ -74,7 +74,8 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
                uint32_t first_n, bool need_all_inputs, bool overlapped) {
     Plan pl{};
     const uint32_t cells = B * F;
-    pl.grid_ok = B <= 65535u && F <= 65535u;
+    // the stream kernel's grid is (slabs, F, B) and its tensor map has a row of F*E bytes
+    pl.grid_ok = B <= 65535u && F <= 65535u && (unsigned long long)F * E < (1ull << 32);
     pl.vec = vector_ok(data, E);
     pl.L = lanes_per_row(E, cells, M, overlapped);
     const uint32_t W = 16u * pl.L;
