@@ -113,8 +113,10 @@ struct AccChain {
     __device__ __forceinline__ void reset() { r = kMagic; s2 = 0.0f; }
     __device__ __forceinline__ void add_c(uint32_t c) {
         const uint32_t r2 = (uint32_t)__dp4a((int)c, (int)c, (int)r);
+#ifndef SK_PROBE_NO_S2                              // experiments only: energy share of the FP32 half
         const float d = __fsub_rn(__uint_as_float(r2), __uint_as_float(r));
         s2 = __fmaf_rn(d, d, s2);
+#endif
         r = r2;
     }
     __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const {
