@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single", "sim", "cm"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
+    ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
+                    help="A/B timing: ldg = the direct-load kernel instead of the TMA stream kernel (sk_debug_set_plan)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -332,6 +334,8 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     sk.lib()
+    if args.path == "ldg":
+        sk.sk_debug_set_plan(sk.SK_PLAN_LDG, 0)
 
     cfg = workload(args.workload)
     K, W = args.steps, max(args.warmup, 3)

@@ -20,7 +20,9 @@
  *     sk_frame_host, which waits for its own copies) and enqueues all work on `stream`
  *     (a cudaStream_t cast to void*; NULL = the legacy default stream) before returning.
  *   - Return value: 0 = enqueued; < 0 = argument error (SK_ERR_*), nothing was enqueued;
- *     > 0 = a cudaError_t reported by a launch or copy.  No exceptions, no global state.
+ *     > 0 = a cudaError_t reported by a launch or copy.  No exceptions.  The only process-wide
+ *     state is the launch counter (sk_launch_count), per-device caches of device attributes, and
+ *     the test-only override of sk_debug_set_plan.
  *   - Receiver selection ("total number of receivers"): `subset` is NULL or E
  *     bytes on the device (non-zero = combine this input).  With subset == NULL the first
  *     `first_n` inputs are combined (first_n = E for the whole array).  N is the number of
@@ -76,29 +78,51 @@ size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M);
 /* Bits of sk_frame's `flags`. */
 #define SK_FRAME_ZERO_FLAGGED  1  /* a8: excise flagged cells in place */
 #define SK_FRAME_INPUTS_READY  2  /* see below */
+#define SK_FRAME_EQ13          4  /* SK = the un-rescaled estimator of PAPER.md:97-104 Eq. 13,
+                                   * (MN+1)/(MN-1) * (S2bar/(MN) - 1), instead of Eq. 14; the flag
+                                   * interval is applied to it unchanged (pass the matching sk_mean) */
 
 /* a1-a8 in one pass over HBM.  Writes SK and mask [T/M][F]; S1_opt / S2_opt [T/M][F][E] are
  * written when non-NULL.  With SK_FRAME_ZERO_FLAGGED every byte (all E inputs, all M rows) of
- * each flagged cell is overwritten in place with 0x88 after the mask is known (the mask and SK
- * are those of the data before excision); otherwise `data` is only read.
- * SK_FRAME_INPUTS_READY is a promise by the caller that `data` and `subset` are not written by
- * the work enqueued on `stream` immediately before this call (e.g. the frame was uploaded and
- * synchronised earlier, or lives in a buffer other than the one the previous call excised).
- * The kernel is launched with programmatic stream serialization; with the promise it reads
- * `data` while the previous kernel on the stream is still draining and waits for it only before
- * its first write (outputs and workspace), so back-to-back frames overlap tail and ramp-up.
- * Without the flag the kernel waits for the previous work before its first read.  Results are
- * identical either way. */
+ * each flagged cell is overwritten in place with 0x88 as soon as the cell's mask is known, by
+ * the same kernel (the mask and SK are those of the data before excision); otherwise `data` is
+ * only read.
+ * SK_FRAME_INPUTS_READY is a promise by the caller that nothing enqueued on `stream` since the
+ * last stream synchronisation or the last sk_frame call made WITHOUT this flag writes this
+ * call's `data` or `subset` (e.g. the frame was uploaded and synchronised earlier, and the calls
+ * in between worked on, and excised, other buffers).  The kernel is launched with programmatic
+ * stream serialization; with the promise it reads `data` while the previous kernel on the stream
+ * is still draining and waits for it only before its first write (outputs and workspace), so
+ * back-to-back frames overlap tail and ramp-up.  Without the flag the kernel waits for all
+ * previous work on the stream before its first read.  Results are identical either way. */
 int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
              const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
              int flags, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
              void* workspace, size_t workspace_bytes, void* stream);
 
+/* Several integration lengths from ONE pass over HBM ("compute real-time SK
+ * estimates at a variety of integration lengths"): the fused path at M, 2M, ..., M << (nlev-1),
+ * 1 <= nlev <= 4.  Eq. 7's sums over 2M samples are the sums of two adjacent M-sample blocks
+ * (exact integers), so the data is streamed once and every length gets its own Eq. 14 estimate
+ * and flag decision.  h_SK / h_mask / h_sk_means are HOST arrays of nlev entries: device
+ * pointers SK_l float32 [T/(M<<l)][F] and mask_l uint8 [T/(M<<l)][F], and the flag centre of each
+ * length.  T % (M << (nlev-1)) == 0 and M << (nlev-1) <= 65536.  Workspace: the size
+ * sk_frame_multi_workspace_bytes returns, zero-filled before first use, left zero-filled.
+ * With SK_FRAME_ZERO_FLAGGED a sample is excised when the cell of ANY length that contains it is
+ * flagged; every estimate is that of the data before excision.  Other flags as for sk_frame. */
+size_t sk_frame_multi_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev);
+int sk_frame_multi(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev,
+                   const uint8_t* subset, uint32_t first_n, float n_sigma, const float* h_sk_means,
+                   int flags, float* const* h_SK, uint8_t* const* h_mask,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
 /* End-to-end form with HOST buffers (pinned memory recommended): copies h_data to d_data,
  * runs sk_frame there, copies SK and mask (and, with SK_FRAME_ZERO_FLAGGED, the excised data) back, and
  * waits for the copies.  d_data (T*F*E bytes), d_SK, d_mask, workspace are caller-owned device
  * buffers; subset is a device pointer as above.  h_data is written only with SK_FRAME_ZERO_FLAGGED;
- * SK_FRAME_INPUTS_READY is ignored (the upload precedes the kernel). */
+ * SK_FRAME_INPUTS_READY is ignored (the upload precedes the kernel).  Argument errors (< 0) are
+ * reported before anything is enqueued; after a launch or copy error (> 0) the call still waits
+ * for what it had enqueued. */
 int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
                   const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
                   int flags, float* h_SK, uint8_t* h_mask,
@@ -162,6 +186,14 @@ int sk_version(void);
 /* Number of kernels the library has launched in this process so far (for the bench's
  * gpu_launches count; monotonically increasing, thread-safe). */
 unsigned long long sk_launch_count(void);
+
+/* Tests and A/B timing only: override the kernel choice of the fused path for the whole process.
+ * path = SK_PLAN_AUTO (default) or SK_PLAN_LDG (direct-load kernel instead of the TMA stream
+ * kernel); lanes = 0 (automatic) or 1, 2, 4, 8, 16: slab width 16*lanes inputs, if not wider than
+ * the automatic choice.  Results do not depend on either. */
+#define SK_PLAN_AUTO 0
+#define SK_PLAN_LDG  1
+void sk_debug_set_plan(int path, int lanes);
 
 #ifdef __cplusplus
 }

@@ -14,9 +14,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
-           "sk_frame_host", "sk_rebin_sums", "sk_single", "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments",
-           "sk_strerror", "sk_version",
-           "sk_launch_count")
+           "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
+           "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
+           "sk_launch_count", "sk_debug_set_plan")
+
+# bits of sk_frame's `flags` (include/sk_b200.h)
+SK_FRAME_ZERO_FLAGGED, SK_FRAME_INPUTS_READY, SK_FRAME_EQ13 = 1, 2, 4
+SK_PLAN_AUTO, SK_PLAN_LDG = 0, 1
 
 _lib = None
 
@@ -42,6 +46,11 @@ def lib() -> C.CDLL:
     L.sk_frame_workspace_bytes.restype = sz
     L.sk_frame.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, sz, vp]
     L.sk_frame_host.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_frame_multi_workspace_bytes.argtypes = [u32, u32, u32, u32, u32]
+    L.sk_frame_multi_workspace_bytes.restype = sz
+    L.sk_frame_multi.argtypes = [vp, u32, u32, u32, u32, u32, vp, u32, f32, vp, i32, vp, vp, vp, sz, vp]
+    L.sk_debug_set_plan.argtypes = [i32, i32]
+    L.sk_debug_set_plan.restype = None
     L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
@@ -52,7 +61,7 @@ def lib() -> C.CDLL:
     L.sk_strerror.restype = C.c_char_p
     L.sk_version.restype = i32
     L.sk_launch_count.restype = C.c_ulonglong
-    for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_host", "sk_rebin_sums",
+    for name in ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums",
                  "sk_single", "sk_significance", "sk_sim_digitised", "sk_moments", "sk_sim_common_mode"):
         getattr(L, name).restype = i32
     _lib = L
@@ -71,6 +80,12 @@ def sk_launch_count() -> int:
     return int(lib().sk_launch_count())
 
 
+def sk_debug_set_plan(path: int = SK_PLAN_AUTO, lanes: int = 0) -> None:
+    """Tests and A/B timing only (include/sk_b200.h): force the direct-load kernel and / or a
+    narrower slab width for the whole process.  (0, 0) restores the automatic choice."""
+    lib().sk_debug_set_plan(int(path), int(lanes))
+
+
 def _check(rc: int, what: str):
     if rc != 0:
         raise SKError(f"{what} failed ({rc}): {sk_strerror(rc)}")
@@ -84,15 +99,30 @@ def _dev(t: torch.Tensor, dtype, what: str) -> torch.Tensor:
     return t
 
 
-def _stream(stream) -> int:
+def _cur() -> int:
+    """The raw handle of torch's current stream (inside `with torch.cuda.stream(...)`)."""
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _torch_stream(stream, device):
+    """The torch.cuda.Stream the call will run on (a raw handle is wrapped): temporaries are
+    allocated, filled and released in its order, so the caching allocator cannot hand them to
+    another stream while the kernel is pending."""
     if stream is None:
-        return torch.cuda.current_stream().cuda_stream
-    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+        return torch.cuda.current_stream(device)
+    if isinstance(stream, torch.cuda.Stream):
+        return stream
+    return torch.cuda.ExternalStream(int(stream), device=device)
 
 
 def _subset(subset, E, device):
+    """Receiver subset -> E bytes on the device (uploaded on the current stream: callers hold
+    `with torch.cuda.stream(...)` around this and the launch)."""
     if subset is None:
         return None
+    if (isinstance(subset, torch.Tensor) and subset.is_cuda and subset.dtype == torch.uint8
+            and subset.is_contiguous() and tuple(subset.shape) == (E,)):
+        return subset
     s = torch.as_tensor(subset)
     s = (s != 0).to(torch.uint8).to(device).contiguous()
     if s.shape != (E,):
@@ -118,10 +148,17 @@ def sk_frame_workspace_bytes(T: int, F: int, E: int, M: int) -> int:
     return int(lib().sk_frame_workspace_bytes(T, F, E, M))
 
 
-def workspace_for(T, F, E, M, device, stream_id=0) -> torch.Tensor:
-    """A zero-filled device workspace for sk_frame, cached per (device, stream, size).  The library
-    leaves a workspace zero-filled after every call, so it is cleared only when created."""
-    n = sk_frame_workspace_bytes(T, F, E, M)
+def sk_frame_multi_workspace_bytes(T: int, F: int, E: int, M: int, nlev: int) -> int:
+    return int(lib().sk_frame_multi_workspace_bytes(T, F, E, M, nlev))
+
+
+def workspace_for(T, F, E, M, device, stream_id=0, nlev=1) -> torch.Tensor:
+    """A zero-filled device workspace for sk_frame / sk_frame_multi, cached per (device, stream,
+    size).  The library leaves a workspace zero-filled after every call, so it is cleared only
+    when created — on the CURRENT torch stream: call this under `with torch.cuda.stream(s)` for
+    the stream s the workspace will be used on (sk_frame does), and never use one workspace on
+    two streams."""
+    n = sk_frame_multi_workspace_bytes(T, F, E, M, nlev)
     if n == 0:
         raise SKError("bad shape for sk_frame")
     key = (str(device), stream_id, n)
@@ -135,70 +172,75 @@ def workspace_for(T, F, E, M, device, stream_id=0) -> torch.Tensor:
 def sk_power_sums(data: torch.Tensor, M: int, stream=None):
     """PAPER.md:77 Eq. 7.  data uint8 [T][F][E] (CUDA) -> S1, S2 uint32 [T/M][F][E]."""
     _dev(data, torch.uint8, "data")
-    T, F, E = data.shape
-    B = T // M if M else 0
-    S1 = torch.empty((B, F, E), dtype=torch.uint32, device=data.device)
-    S2 = torch.empty_like(S1)
-    _check(lib().sk_power_sums(data.data_ptr(), T, F, E, M, S1.data_ptr(), S2.data_ptr(), _stream(stream)),
-           "sk_power_sums")
-    return S1, S2
+    with torch.cuda.stream(_torch_stream(stream, data.device)):   # outputs are allocated in stream order
+        T, F, E = data.shape
+        B = T // M if M else 0
+        S1 = torch.empty((B, F, E), dtype=torch.uint32, device=data.device)
+        S2 = torch.empty_like(S1)
+        _check(lib().sk_power_sums(data.data_ptr(), T, F, E, M, S1.data_ptr(), S2.data_ptr(), _cur()), "sk_power_sums")
+        return S1, S2
 
 
 def sk_combine(S1: torch.Tensor, S2: torch.Tensor, M: int, subset=None, first_n=None, stream=None):
     """PAPER.md:84-88 Eq. 9-11, :108-113 Eq. 14.  S1, S2 uint32 [B][F][E] -> SK float32 [B][F]."""
     _dev(S1, torch.uint32, "S1")
     _dev(S2, torch.uint32, "S2")
-    B, F, E = S1.shape
-    sub = _subset(subset, E, S1.device)
-    if sub is None and first_n is None:
-        first_n = E
-    SK = torch.empty((B, F), dtype=torch.float32, device=S1.device)
-    _check(lib().sk_combine(S1.data_ptr(), S2.data_ptr(), B, F, E, M, _ptr(sub), int(first_n or 0),
-                            SK.data_ptr(), _stream(stream)), "sk_combine")
-    return SK
+    with torch.cuda.stream(_torch_stream(stream, S1.device)):   # outputs are allocated in stream order
+        B, F, E = S1.shape
+        sub = _subset(subset, E, S1.device)
+        if sub is None and first_n is None:
+            first_n = E
+        SK = torch.empty((B, F), dtype=torch.float32, device=S1.device)
+        _check(lib().sk_combine(S1.data_ptr(), S2.data_ptr(), B, F, E, M, _ptr(sub), int(first_n or 0),
+                                SK.data_ptr(), _cur()), "sk_combine")
+        return SK
 
 
 def sk_flag(SK: torch.Tensor, M: int, N: int, n_sigma: float, sk_mean: float = 1.0, stream=None):
     """PAPER.md:183 / :119 Eq. 16.  SK float32 [B][F] -> mask uint8 [B][F]."""
     _dev(SK, torch.float32, "SK")
-    B, F = SK.shape
-    mask = torch.empty((B, F), dtype=torch.uint8, device=SK.device)
-    _check(lib().sk_flag(SK.data_ptr(), B, F, M, N, n_sigma, sk_mean, mask.data_ptr(), _stream(stream)),
-           "sk_flag")
-    return mask
+    with torch.cuda.stream(_torch_stream(stream, SK.device)):   # outputs are allocated in stream order
+        B, F = SK.shape
+        mask = torch.empty((B, F), dtype=torch.uint8, device=SK.device)
+        _check(lib().sk_flag(SK.data_ptr(), B, F, M, N, n_sigma, sk_mean, mask.data_ptr(), _cur()),
+               "sk_flag")
+        return mask
 
 
 def sk_rebin_sums(S1: torch.Tensor, S2: torch.Tensor, M: int, factor: int, stream=None):
     """sums at block length M re-binned to M*factor.  [B][F][E] -> [B/factor][F][E]."""
     _dev(S1, torch.uint32, "S1")
     _dev(S2, torch.uint32, "S2")
-    B, F, E = S1.shape
-    Bo = B // factor if factor else 0
-    O1 = torch.empty((Bo, F, E), dtype=torch.uint32, device=S1.device)
-    O2 = torch.empty_like(O1)
-    _check(lib().sk_rebin_sums(S1.data_ptr(), S2.data_ptr(), B, F, E, M, factor, O1.data_ptr(), O2.data_ptr(),
-                               _stream(stream)), "sk_rebin_sums")
-    return O1, O2
+    with torch.cuda.stream(_torch_stream(stream, S1.device)):   # outputs are allocated in stream order
+        B, F, E = S1.shape
+        Bo = B // factor if factor else 0
+        O1 = torch.empty((Bo, F, E), dtype=torch.uint32, device=S1.device)
+        O2 = torch.empty_like(O1)
+        _check(lib().sk_rebin_sums(S1.data_ptr(), S2.data_ptr(), B, F, E, M, factor, O1.data_ptr(), O2.data_ptr(),
+                                   _cur()), "sk_rebin_sums")
+        return O1, O2
 
 
 def sk_single(S1: torch.Tensor, S2: torch.Tensor, M: int, stream=None):
     """PAPER.md:80 Eq. 8 per receiver.  S1, S2 uint32 [B][F][E] -> SKi float32 [B][F][E]."""
     _dev(S1, torch.uint32, "S1")
     _dev(S2, torch.uint32, "S2")
-    B, F, E = S1.shape
-    SKi = torch.empty((B, F, E), dtype=torch.float32, device=S1.device)
-    _check(lib().sk_single(S1.data_ptr(), S2.data_ptr(), B, F, E, M, SKi.data_ptr(), _stream(stream)), "sk_single")
-    return SKi
+    with torch.cuda.stream(_torch_stream(stream, S1.device)):   # outputs are allocated in stream order
+        B, F, E = S1.shape
+        SKi = torch.empty((B, F, E), dtype=torch.float32, device=S1.device)
+        _check(lib().sk_single(S1.data_ptr(), S2.data_ptr(), B, F, E, M, SKi.data_ptr(), _cur()), "sk_single")
+        return SKi
 
 
 def sk_significance(SK: torch.Tensor, M: int, N: int, sk_mean: float = 1.0, stream=None):
     """PAPER.md:183 detection significance.  SK float32 [B][F] -> float32 [B][F]."""
     _dev(SK, torch.float32, "SK")
-    B, F = SK.shape
-    sig = torch.empty((B, F), dtype=torch.float32, device=SK.device)
-    _check(lib().sk_significance(SK.data_ptr(), B, F, M, N, sk_mean, sig.data_ptr(), _stream(stream)),
-           "sk_significance")
-    return sig
+    with torch.cuda.stream(_torch_stream(stream, SK.device)):   # outputs are allocated in stream order
+        B, F = SK.shape
+        sig = torch.empty((B, F), dtype=torch.float32, device=SK.device)
+        _check(lib().sk_significance(SK.data_ptr(), B, F, M, N, sk_mean, sig.data_ptr(), _cur()),
+               "sk_significance")
+        return sig
 
 
 def sk_sim_digitised(T: int, F: int, E: int, thr: torch.Tensor, seed: int, frame: int = 0, out=None, stream=None):
@@ -207,63 +249,111 @@ def sk_sim_digitised(T: int, F: int, E: int, thr: torch.Tensor, seed: int, frame
     _dev(thr, torch.uint32, "thr")
     if tuple(thr.shape) != (E, 14):
         raise SKError("thr must be [E][14]")
-    if out is None:
-        out = torch.empty((T, F, E), dtype=torch.uint8, device=thr.device)
-    _dev(out, torch.uint8, "out")
-    _check(lib().sk_sim_digitised(out.data_ptr(), T, F, E, thr.data_ptr(), seed, frame, _stream(stream)),
-           "sk_sim_digitised")
-    return out
+    with torch.cuda.stream(_torch_stream(stream, thr.device)):   # outputs are allocated in stream order
+        if out is None:
+            out = torch.empty((T, F, E), dtype=torch.uint8, device=thr.device)
+        _dev(out, torch.uint8, "out")
+        _check(lib().sk_sim_digitised(out.data_ptr(), T, F, E, thr.data_ptr(), seed, frame, _cur()),
+               "sk_sim_digitised")
+        return out
 
 
 def sk_sim_common_mode(D: int, M: int, N: int, amp: float, seed: int, device="cuda", stream=None):
     """PAPER.md:262-272 (App. A): SK~ of D simulated datasets (M samples x N receivers, common-mode
     amplitude amp): float32 [D][1] on `device` (shape ready for sk_moments)."""
-    SK = torch.empty((D, 1), dtype=torch.float32, device=device)
-    if not SK.is_cuda:
+    dev = torch.device(device)
+    if dev.type != "cuda":
         raise SKError("sk_sim_common_mode needs a CUDA device (there is no CPU fallback)")
-    _check(lib().sk_sim_common_mode(D, M, N, float(amp), seed, SK.data_ptr(), _stream(stream)), "sk_sim_common_mode")
-    return SK
+    with torch.cuda.stream(_torch_stream(stream, dev)):
+        SK = torch.empty((D, 1), dtype=torch.float32, device=dev)
+        _check(lib().sk_sim_common_mode(D, M, N, float(amp), seed, SK.data_ptr(), _cur()), "sk_sim_common_mode")
+        return SK
 
 
 def sk_moments(SK: torch.Tensor, stream=None):
     """Mean and unbiased variance of SK float32 [B][F] over the blocks: float64 [F] each."""
     _dev(SK, torch.float32, "SK")
-    B, F = SK.shape
-    mean = torch.empty(F, dtype=torch.float64, device=SK.device)
-    var = torch.empty(F, dtype=torch.float64, device=SK.device)
-    _check(lib().sk_moments(SK.data_ptr(), B, F, mean.data_ptr(), var.data_ptr(), _stream(stream)), "sk_moments")
-    return mean, var
+    with torch.cuda.stream(_torch_stream(stream, SK.device)):   # outputs are allocated in stream order
+        B, F = SK.shape
+        mean = torch.empty(F, dtype=torch.float64, device=SK.device)
+        var = torch.empty(F, dtype=torch.float64, device=SK.device)
+        _check(lib().sk_moments(SK.data_ptr(), B, F, mean.data_ptr(), var.data_ptr(), _cur()), "sk_moments")
+        return mean, var
 
 
 def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: float = 3.0,
              sk_mean: float = 1.0, zero_flagged: bool = False, want_sums: bool = False,
              out: Optional[SKResult] = None, workspace: Optional[torch.Tensor] = None,
-             stream=None, inputs_ready: bool = False) -> SKResult:
+             stream=None, inputs_ready: bool = False, eq13: bool = False) -> SKResult:
     """The fused path (one pass over HBM).  `data` is modified in place only if zero_flagged.
-    inputs_ready = SK_FRAME_INPUTS_READY (include/sk_b200.h): `data`/`subset` are not written by
-    the work enqueued on the stream just before this call, so the kernel may overlap it."""
+    inputs_ready = SK_FRAME_INPUTS_READY (include/sk_b200.h): nothing enqueued on the stream since
+    its last synchronisation (or the last call without the flag) writes `data`/`subset`, so the
+    kernel may overlap the previous one.  eq13 = SK_FRAME_EQ13."""
     _dev(data, torch.uint8, "data")
     T, F, E = data.shape
     B = T // M if M else 0
     dev = data.device
-    sub = subset if (isinstance(subset, torch.Tensor) and subset.is_cuda and subset.dtype == torch.uint8
-                     and subset.is_contiguous() and subset.shape == (E,)) else _subset(subset, E, dev)
-    if sub is None and first_n is None:
-        first_n = E
-    st = _stream(stream)
-    if out is None:
-        SK = torch.empty((B, F), dtype=torch.float32, device=dev)
-        mask = torch.empty((B, F), dtype=torch.uint8, device=dev)
-        S1 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
-        S2 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
-        out = SKResult(SK, mask, S1, S2)
-    if workspace is None:
-        workspace = workspace_for(T, F, E, M, dev, st)
-    _check(lib().sk_frame(data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
-                          (1 if zero_flagged else 0) | (2 if inputs_ready else 0), out.SK.data_ptr(),
-                          out.mask.data_ptr(),
-                          _ptr(out.S1), _ptr(out.S2), workspace.data_ptr(),
-                          workspace.numel() * workspace.element_size(), st), "sk_frame")
+    ts = _torch_stream(stream, dev)
+    with torch.cuda.stream(ts):                 # outputs, subset upload, workspace fill: in stream order
+        sub = _subset(subset, E, dev)
+        if sub is None and first_n is None:
+            first_n = E
+        if out is None:
+            SK = torch.empty((B, F), dtype=torch.float32, device=dev)
+            mask = torch.empty((B, F), dtype=torch.uint8, device=dev)
+            S1 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
+            S2 = torch.empty((B, F, E), dtype=torch.uint32, device=dev) if want_sums else None
+            out = SKResult(SK, mask, S1, S2)
+        if workspace is None:
+            workspace = workspace_for(T, F, E, M, dev, ts.cuda_stream)
+        flags = ((SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_INPUTS_READY if inputs_ready else 0)
+                 | (SK_FRAME_EQ13 if eq13 else 0))
+        _check(lib().sk_frame(data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
+                              flags, out.SK.data_ptr(), out.mask.data_ptr(), _ptr(out.S1), _ptr(out.S2),
+                              workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                              ts.cuda_stream), "sk_frame")
+    return out
+
+
+class SKMultiResult(NamedTuple):
+    SK: list        # per integration length M << l: float32 [T / (M << l)][F]
+    mask: list      # uint8, same shapes
+
+
+def sk_frame_multi(data: torch.Tensor, M: int, nlev: int, subset=None, first_n=None, n_sigma: float = 3.0,
+                   sk_means=None, zero_flagged: bool = False, out: Optional[SKMultiResult] = None,
+                   workspace: Optional[torch.Tensor] = None, stream=None,
+                   inputs_ready: bool = False) -> SKMultiResult:
+    """SK and mask at the integration lengths M, 2M, ..., M << (nlev-1) from one
+    pass over the data.  sk_means: one flag centre per length (default 1.0 each)."""
+    _dev(data, torch.uint8, "data")
+    T, F, E = data.shape
+    dev = data.device
+    nlev = int(nlev)
+    if not 1 <= nlev <= 4:
+        raise SKError("nlev must be in [1, 4]")
+    means = [1.0] * nlev if sk_means is None else [float(x) for x in sk_means]
+    if len(means) != nlev:
+        raise SKError("sk_means must have nlev entries")
+    ts = _torch_stream(stream, dev)
+    with torch.cuda.stream(ts):
+        sub = _subset(subset, E, dev)
+        if sub is None and first_n is None:
+            first_n = E
+        if out is None:
+            shapes = [((T // (M << l)) if M else 0, F) for l in range(nlev)]
+            out = SKMultiResult([torch.empty(s, dtype=torch.float32, device=dev) for s in shapes],
+                                [torch.empty(s, dtype=torch.uint8, device=dev) for s in shapes])
+        if workspace is None:
+            workspace = workspace_for(T, F, E, M, dev, ts.cuda_stream, nlev)
+        c_means = (C.c_float * nlev)(*means)
+        c_SK = (C.c_void_p * nlev)(*[t.data_ptr() for t in out.SK])
+        c_mask = (C.c_void_p * nlev)(*[t.data_ptr() for t in out.mask])
+        flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_INPUTS_READY if inputs_ready else 0)
+        _check(lib().sk_frame_multi(data.data_ptr(), T, F, E, M, nlev, _ptr(sub), int(first_n or 0), n_sigma,
+                                    C.cast(c_means, C.c_void_p), flags, C.cast(c_SK, C.c_void_p),
+                                    C.cast(c_mask, C.c_void_p), workspace.data_ptr(),
+                                    workspace.numel() * workspace.element_size(), ts.cuda_stream), "sk_frame_multi")
     return out
 
 
@@ -276,14 +366,15 @@ def sk_frame_host(h_data: torch.Tensor, M: int, h_SK: torch.Tensor, h_mask: torc
         raise SKError("h_* tensors must live in host memory")
     T, F, E = h_data.shape
     _dev(d_data, torch.uint8, "d_data")
-    sub = _subset(subset, E, d_data.device)
-    if sub is None and first_n is None:
-        first_n = E
-    st = _stream(stream)
-    if workspace is None:
-        workspace = workspace_for(T, F, E, M, d_data.device, st)
-    _check(lib().sk_frame_host(h_data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma,
-                               sk_mean, int(bool(zero_flagged)), h_SK.data_ptr(), h_mask.data_ptr(),
-                               d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
-                               workspace.numel() * workspace.element_size(), st), "sk_frame_host")
+    ts = _torch_stream(stream, d_data.device)
+    with torch.cuda.stream(ts):
+        sub = _subset(subset, E, d_data.device)
+        if sub is None and first_n is None:
+            first_n = E
+        if workspace is None:
+            workspace = workspace_for(T, F, E, M, d_data.device, ts.cuda_stream)
+        _check(lib().sk_frame_host(h_data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma,
+                                   sk_mean, int(bool(zero_flagged)), h_SK.data_ptr(), h_mask.data_ptr(),
+                                   d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
+                                   workspace.numel() * workspace.element_size(), ts.cuda_stream), "sk_frame_host")
     return h_SK, h_mask

@@ -33,7 +33,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "--shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += os.environ.get("SK_B200_NVCC_FLAGS", "").split()     # e.g. -DSK_NWIDE=1 for A/B experiments
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)

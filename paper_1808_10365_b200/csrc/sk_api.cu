@@ -3,7 +3,6 @@
 #include <atomic>
 #include <cmath>
 #include <cstdint>
-#include <cstdlib>
 #include <cstring>
 
 #include "../../include/sk_b200.h"
@@ -11,19 +10,37 @@
 #include "sk_tma.cuh"
 #include "sk_sim.cuh"
 
-#include <cstdlib>
-#include <cstring>
-
 namespace {
 
 std::atomic<unsigned long long> g_launches{0};
+// sk_debug_set_plan (tests and A/B timing only): 0 = automatic
+std::atomic<int> g_force_path{0};     // SK_PLAN_LDG: never the stream kernel
+std::atomic<int> g_force_lanes{0};    // a (narrower) slab width of 16 * lanes inputs
 
 inline int launch_status() {
     const cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SK_OK : (int)e;
 }
 
-int sm_count();
+constexpr int kMaxDevices = 64;
+
+int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+    return dev;
+}
+
+int sm_count() {
+    static std::atomic<int> cache[kMaxDevices];
+    const int dev = current_device();
+    int v = cache[dev].load(std::memory_order_relaxed);
+    if (v == 0) {
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+        (void)cudaGetLastError();
+        cache[dev].store(v, std::memory_order_relaxed);
+    }
+    return v;
+}
 
 // Lanes per row for the vector path (slab width = 16*L inputs).  The sum over inputs follows a
 // canonical tree over the input indices (sk_kernels.cuh), so the choice affects speed only, never
@@ -31,19 +48,14 @@ int sm_count();
 // SM enough warps; otherwise narrower slabs.  A lone frame needs ~16 warps per SM of its own;
 // frames that overlap their neighbours on the stream (SK_FRAME_INPUTS_READY) share the SM with
 // them and run best on wide slabs from 8 warps per SM up (measured on config 1: 16.3 vs 17.0 us).
-inline int lanes_per_row(uint32_t E, uint32_t cells, uint32_t M, bool overlapped) {
+inline int lanes_per_row(uint32_t E, unsigned long long units_per_slab_column, bool overlapped) {
     const uint32_t vecs = E / 16;            // 128-bit vectors per row
     int L = 16;
     while (L > 1 && (uint32_t)L > vecs) L >>= 1;
     const unsigned long long want = (unsigned long long)sm_count() * (overlapped ? 8u : 16u);
-    while (L > 4 && (unsigned long long)cells * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
-    if (const char* e = std::getenv("SK_B200_LANES")) {     // tests: force a (narrower) slab width
-        const int v = std::atoi(e);
-        if (v >= 1 && v <= L && (v & (v - 1)) == 0) L = v;
-    }
-    // long blocks: narrower slabs put more rows under one warp-wide read, so that a lane still
-    // adds at most AccChain::kMaxSamples samples per unit (the stream kernel's exactness limit)
-    while (L > 1 && (M + 32u / L - 1) / (32u / L) > sk::AccChain::kMaxSamples) L >>= 1;
+    while (L > 4 && units_per_slab_column * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
+    const int v = g_force_lanes.load(std::memory_order_relaxed);
+    if (v >= 1 && v <= L && (v & (v - 1)) == 0) L = v;
     return L;
 }
 
@@ -61,44 +73,67 @@ int check_shape(uint32_t T, uint32_t F, uint32_t E, uint32_t M) {
     return SK_OK;
 }
 
+// Rows per accumulator read-out of the stream kernel: the largest divisor of M that is a whole
+// number of TMA tiles and keeps a lane within AccChain2's 128 samples (rows <= 128 * RPW).
+// 0 = none (ragged or very short blocks): the direct-load kernel runs instead.
+uint32_t chunk_rows(uint32_t M, int L) {
+    const uint32_t RPW = 32u / L, cap = sk::AccChain2::kMaxSamples * RPW;
+    const uint32_t R = sk::kTileBytes / (16u * L);
+    if (M % R) return 0;
+    for (uint32_t d = (M < cap ? M : cap) / R * R; d >= R; d -= R)
+        if (M % d == 0) return d >= cap / 4 || d == M ? d : 0;
+    return 0;
+}
+
 struct Plan {
     bool vec;
     int L;
     uint32_t slabs;       // launched slabs per cell
-    bool wide;            // AccWide usable (samples per lane <= 511)
-    bool stream;          // stream kernel usable (samples per lane <= 128)
-    bool grid_ok;         // F and B fit the y and z grid dimensions
+    bool wide;            // AccWide2 usable by the direct-load kernel (samples per lane <= 511)
+    bool chain;           // AccChain2 usable by the direct-load kernel (samples per lane <= 128)
+    uint32_t chunk;       // stream kernel: rows per read-out, 0 = stream kernel not usable
+    uint32_t bpu;         // stream kernel: M-row blocks per unit (a power of two dividing B, >= 1 << (nlev-1))
 };
 
+// nlev = integration lengths wanted (M << 0 .. M << (nlev-1)); B % (1 << (nlev-1)) == 0.
 Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F, const uint8_t* subset,
-               uint32_t first_n, bool need_all_inputs, bool overlapped) {
+               uint32_t first_n, bool need_all_inputs, bool overlapped, uint32_t nlev) {
     Plan pl{};
-    const uint32_t cells = B * F;
-    // the stream kernel's grid is (slabs, F, B) and its tensor map has a row of F*E bytes
-    pl.grid_ok = B <= 65535u && F <= 65535u && (unsigned long long)F * E < (1ull << 32);
     pl.vec = vector_ok(data, E);
-    pl.L = lanes_per_row(E, cells, M, overlapped);
+    // blocks per unit: the longest length's worth, and for short blocks as many as make a unit
+    // of >= 256 rows while every SM still gets its share of units
+    uint32_t bpu = 1u << (nlev - 1);
+    const unsigned long long want = (unsigned long long)sm_count() * 48u;
+    while (M * bpu < 256u && B % (2u * bpu) == 0 &&
+           (unsigned long long)(B / (2u * bpu)) * F * ((E + 255u) / 256u) >= want)
+        bpu *= 2u;
+    pl.bpu = bpu;
+    pl.L = lanes_per_row(E, (unsigned long long)(B / bpu) * F, overlapped);
     const uint32_t W = 16u * pl.L;
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
     pl.slabs = (cover + W - 1) / W;
     const uint32_t RPW = 32u / pl.L;
     const uint32_t iters = (M + RPW - 1) / RPW;
-    pl.wide = iters <= sk::AccWide::kMaxSamples;
-    pl.stream = iters <= sk::AccChain::kMaxSamples;
+    pl.wide = iters <= sk::AccWide2::kMaxSamples;
+    pl.chain = iters <= sk::AccChain2::kMaxSamples;
+    // the stream kernel's grid is (slabs, F, B / bpu) and its tensor map has a row of F*E bytes
+    const bool grid_ok = B / bpu <= 65535u && F <= 65535u && (unsigned long long)F * E < (1ull << 32) &&
+                         (unsigned long long)B * M < (1ull << 31);
+    pl.chunk = (pl.vec && grid_ok && pl.L >= 4) ? chunk_rows(M, pl.L) : 0u;
     return pl;
 }
 
-template <class Acc>
+template <class Acc2>
 void launch_vec_L(int L, const sk::FrameParams& p, cudaStream_t st) {
     const unsigned grid = (p.nunits + sk::kWarpsPerCta - 1) / sk::kWarpsPerCta;
     const unsigned block = sk::kWarpsPerCta * 32;
     switch (L) {
-        case 16: sk::sk_frame_kernel<16, Acc><<<grid, block, 0, st>>>(p); break;
-        case 8:  sk::sk_frame_kernel<8, Acc><<<grid, block, 0, st>>>(p); break;
-        case 4:  sk::sk_frame_kernel<4, Acc><<<grid, block, 0, st>>>(p); break;
-        case 2:  sk::sk_frame_kernel<2, Acc><<<grid, block, 0, st>>>(p); break;
-        default: sk::sk_frame_kernel<1, Acc><<<grid, block, 0, st>>>(p); break;
+        case 16: sk::sk_frame_kernel<16, Acc2><<<grid, block, 0, st>>>(p); break;
+        case 8:  sk::sk_frame_kernel<8, Acc2><<<grid, block, 0, st>>>(p); break;
+        case 4:  sk::sk_frame_kernel<4, Acc2><<<grid, block, 0, st>>>(p); break;
+        case 2:  sk::sk_frame_kernel<2, Acc2><<<grid, block, 0, st>>>(p); break;
+        default: sk::sk_frame_kernel<1, Acc2><<<grid, block, 0, st>>>(p); break;
     }
     ++g_launches;
 }
@@ -122,36 +157,26 @@ EncodeTiledFn encode_tiled() {
     return fn;
 }
 
-int sm_count() {
-    static int n = [] {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            v = 148;
-        return v > 0 ? v : 148;
-    }();
-    return n;
+// The stream kernel runs whenever it applies; sk_debug_set_plan(SK_PLAN_LDG, ..) turns it off.
+bool stream_wanted(const Plan& pl) {
+    if (g_force_path.load(std::memory_order_relaxed) == SK_PLAN_LDG) return false;
+    return pl.chunk != 0 && encode_tiled() != nullptr;
 }
 
-// SK_B200_PATH=ldg|tma forces one vector kernel (for tests and A/B timing); default: TMA when it applies
-// (the stream kernel keeps its sums in AccWide fields: at most 511 samples per lane and unit).
-bool tma_wanted(const Plan& pl) {
-    const char* e = std::getenv("SK_B200_PATH");
-    if (e && std::strcmp(e, "ldg") == 0) return false;
-    return pl.stream && pl.grid_ok && encode_tiled() != nullptr;
-}
-
-template <int L>
-int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(sk::sk_stream_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+template <int L, int NLEV, bool CHUNKED>
+int launch_stream_K(const CUtensorMap& tmap, const sk::FrameParams& p, uint32_t zblocks, cudaStream_t st) {
+    // per device: the opt-in attributes belong to the device's copy of the function
+    static std::atomic<bool> attr_set[kMaxDevices];
+    const int dev = current_device();
+    if (!attr_set[dev].load(std::memory_order_acquire)) {
+        cudaFuncSetAttribute(sk::sk_stream_kernel<L, NLEV, CHUNKED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)sk::kStreamSmemBytes);
-        cudaFuncSetAttribute(sk::sk_stream_kernel<L>, cudaFuncAttributePreferredSharedMemoryCarveout,
+        cudaFuncSetAttribute(sk::sk_stream_kernel<L, NLEV, CHUNKED>, cudaFuncAttributePreferredSharedMemoryCarveout,
                              cudaSharedmemCarveoutMaxShared);
-        attr_set = true;
+        attr_set[dev].store(true, std::memory_order_release);
     }
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(p.slabs, p.F, p.B);
+    cfg.gridDim = dim3(p.slabs, p.F, zblocks);
     cfg.blockDim = dim3(32);
     cfg.dynamicSmemBytes = sk::kStreamSmemBytes;
     cfg.stream = st;
@@ -160,13 +185,25 @@ int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, cudaStrea
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    const cudaError_t e = cudaLaunchKernelEx(&cfg, sk::sk_stream_kernel<L>, tmap, p);
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, sk::sk_stream_kernel<L, NLEV, CHUNKED>, tmap, p);
     return e == cudaSuccess ? SK_OK : (int)e;
 }
 
-int launch_stream(int L, const sk::FrameParams& p, cudaStream_t st) {
+template <int L>
+int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, bool chunked, uint32_t zblocks,
+                    cudaStream_t st) {
+    switch (p.nlev) {
+        case 1: return chunked ? launch_stream_K<L, 1, true>(tmap, p, zblocks, st)
+                               : launch_stream_K<L, 1, false>(tmap, p, zblocks, st);
+        case 2: return launch_stream_K<L, 2, true>(tmap, p, zblocks, st);
+        case 3: return launch_stream_K<L, 3, true>(tmap, p, zblocks, st);
+        default: return launch_stream_K<L, 4, true>(tmap, p, zblocks, st);
+    }
+}
+
+int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     CUtensorMap tmap;
-    const uint32_t W = 16u * L;
+    const uint32_t W = 16u * pl.L;
     const cuuint64_t gdim[2] = {(cuuint64_t)p.F * p.E, (cuuint64_t)p.T};
     const cuuint64_t gstride[1] = {(cuuint64_t)p.F * p.E};
     const cuuint32_t box[2] = {(cuuint32_t)W, (cuuint32_t)(sk::kTileBytes / W)};
@@ -175,13 +212,13 @@ int launch_stream(int L, const sk::FrameParams& p, cudaStream_t st) {
                                       gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    const bool chunked = pl.chunk != p.M;
+    const uint32_t zblocks = p.B / pl.bpu;
     int rc;
-    switch (L) {
-        case 16: rc = launch_stream_L<16>(tmap, p, st); break;
-        case 8:  rc = launch_stream_L<8>(tmap, p, st); break;
-        case 4:  rc = launch_stream_L<4>(tmap, p, st); break;
-        case 2:  rc = launch_stream_L<2>(tmap, p, st); break;
-        default: rc = launch_stream_L<1>(tmap, p, st); break;
+    switch (pl.L) {
+        case 16: rc = launch_stream_L<16>(tmap, p, chunked, zblocks, st); break;
+        case 8:  rc = launch_stream_L<8>(tmap, p, chunked, zblocks, st); break;
+        default: rc = launch_stream_L<4>(tmap, p, chunked, zblocks, st); break;
     }
     if (rc == SK_OK) ++g_launches;
     return rc;
@@ -192,12 +229,14 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
     if (pl.vec) {
         p.slabs = pl.slabs;
         p.nunits = cells * pl.slabs;
-        if (tma_wanted(pl)) {
-            const int rc = launch_stream(pl.L, p, st);
+        if (stream_wanted(pl)) {
+            p.chunk = pl.chunk;
+            p.bpu = pl.bpu;
+            const int rc = launch_stream(pl, p, st);
             if (rc != SK_OK) return rc;
-        } else if (pl.stream) launch_vec_L<sk::AccChain>(pl.L, p, st);
-        else if (pl.wide) launch_vec_L<sk::AccWide>(pl.L, p, st);
-        else                launch_vec_L<sk::AccPlain>(pl.L, p, st);
+        } else if (pl.chain) launch_vec_L<sk::AccChain2>(pl.L, p, st);
+        else if (pl.wide)  launch_vec_L<sk::AccWide2>(pl.L, p, st);
+        else               launch_vec_L<sk::AccPlain2>(pl.L, p, st);
     } else {
         sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);
         ++g_launches;
@@ -205,8 +244,102 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
     return launch_status();
 }
 
-size_t workspace_bytes(uint32_t cells, uint32_t slabs_max) {
-    return (size_t)cells * slabs_max * sizeof(double) + (size_t)cells * sizeof(uint32_t);
+size_t level_bytes(uint32_t cells, uint32_t slabs_max) {
+    return (size_t)cells * slabs_max * sizeof(double) + (((size_t)cells * sizeof(uint32_t) + 7u) & ~(size_t)7u);
+}
+
+// Workspace of integration length l: partials [cells_l][slabs_max] then counters [cells_l]; the
+// lengths follow one another.  The place of every array depends on the shape alone (not on
+// first_n or on the slab width), so a workspace stays clean across calls.
+size_t workspace_bytes(uint32_t B, uint32_t F, uint32_t E, uint32_t nlev) {
+    size_t n = 0;
+    for (uint32_t l = 0; l < nlev; ++l) n += level_bytes((B >> l) * F, (E + 15u) / 16u);
+    return n;
+}
+
+int check_frame_args(const uint8_t* subset, uint32_t E, uint32_t first_n, float n_sigma, const float* sk_means,
+                     uint32_t nlev, bool with_mask) {
+    if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
+    if (with_mask) {
+        if (!std::isfinite(n_sigma) || n_sigma < 0) return SK_ERR_PARAM;
+        for (uint32_t l = 0; l < nlev; ++l)
+            if (!std::isfinite(sk_means[l])) return SK_ERR_PARAM;
+    }
+    return SK_OK;
+}
+
+// The fused path for nlev integration lengths (sk_frame: nlev = 1).  All argument checks happen
+// before the first launch.
+int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev,
+               const uint8_t* subset, uint32_t first_n, float n_sigma, const float* sk_means, int flags,
+               float* const* SK, uint8_t* const* mask, uint32_t* S1o, uint32_t* S2o, void* workspace,
+               size_t workspace_bytes_given, cudaStream_t st) {
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    const uint32_t B = T / M;
+    if (nlev < 1 || nlev > (uint32_t)sk::kMaxLevels) return SK_ERR_SHAPE;
+    if (B % (1u << (nlev - 1)) != 0) return SK_ERR_SHAPE;
+    if (((unsigned long long)M << (nlev - 1)) > 65536ull) return SK_ERR_M;
+    bool any_mask = false;
+    for (uint32_t l = 0; l < nlev; ++l) {
+        if (!SK[l]) return SK_ERR_NULL;
+        any_mask = any_mask || mask[l] != nullptr;
+    }
+    if ((flags & SK_FRAME_ZERO_FLAGGED) && !mask[0]) return SK_ERR_NULL;
+    if (int rc = check_frame_args(subset, E, first_n, n_sigma, sk_means, nlev, any_mask)) return rc;
+    if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
+    Plan pl = make_plan(data, E, M, B, F, subset, first_n, S1o != nullptr, (flags & SK_FRAME_INPUTS_READY) != 0, nlev);
+    if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
+    sk::FrameParams p{};
+    p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = B;
+    p.excise = (flags & SK_FRAME_ZERO_FLAGGED) ? const_cast<uint8_t*>(data) : nullptr;
+    p.subset = subset; p.first_n = subset ? 0 : first_n;
+    p.n_sigma = n_sigma;
+    p.nlev = nlev;
+    p.eq13 = (flags & SK_FRAME_EQ13) ? 1u : 0u;
+    p.inputs_ready = (flags & SK_FRAME_INPUTS_READY) ? 1u : 0u;
+    p.S1out = S1o; p.S2out = S2o;
+    const bool one_launch = nlev == 1 || (pl.vec && stream_wanted(pl));
+    if (pl.vec) {
+        if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) ||
+            workspace_bytes_given < workspace_bytes(B, F, E, nlev))
+            return SK_ERR_WORKSPACE;
+    }
+    const uint32_t slabs_max = (E + 15u) / 16u;
+    uint8_t* ws = static_cast<uint8_t*>(workspace);
+    for (uint32_t l = 0; l < nlev; ++l) {
+        const uint32_t cells = (B >> l) * F;
+        p.lev[l].SK = SK[l];
+        p.lev[l].mask = mask[l];
+        p.lev[l].sk_mean = sk_means[l];
+        if (pl.vec) {
+            p.lev[l].partial = reinterpret_cast<double*>(ws);
+            p.lev[l].counter = reinterpret_cast<uint32_t*>(ws + (size_t)cells * slabs_max * sizeof(double));
+            ws += level_bytes(cells, slabs_max);
+        }
+    }
+    if (one_launch) return launch_cells(pl, p, st);
+    // several lengths without the stream kernel: one pass of the fused path per length, then the
+    // excision of every flagged cell of every length (all lengths see the data before excision)
+    for (uint32_t l = 0; l < nlev; ++l) {
+        sk::FrameParams pl_l = p;
+        pl_l.M = M << l; pl_l.B = B >> l; pl_l.nlev = 1; pl_l.excise = nullptr;
+        pl_l.lev[0] = p.lev[l];
+        pl_l.S1out = l == 0 ? S1o : nullptr; pl_l.S2out = l == 0 ? S2o : nullptr;
+        pl_l.inputs_ready = l == 0 ? p.inputs_ready : 0u;
+        Plan q = make_plan(data, E, M << l, B >> l, F, subset, first_n, pl_l.S1out != nullptr, false, 1);
+        q.vec = pl.vec;
+        if (int rc = launch_cells(q, pl_l, st)) return rc;
+    }
+    for (uint32_t l = 0; l < nlev && p.excise; ++l) {
+        if (!mask[l]) continue;
+        const uint32_t Ml = M << l;
+        const dim3 grid((B >> l) * F, (Ml + sk::kExciseRows - 1) / sk::kExciseRows);
+        if (pl.vec) sk::sk_excise_kernel<true><<<grid, 256, 0, st>>>(p, mask[l], Ml);
+        else        sk::sk_excise_kernel<false><<<grid, 256, 0, st>>>(p, mask[l], Ml);
+        ++g_launches;
+        if (int rc = launch_status()) return rc;
+    }
+    return SK_OK;
 }
 
 }  // namespace
@@ -217,51 +350,24 @@ int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint3
                   uint32_t* S1, uint32_t* S2, void* stream) {
     if (!data || !S1 || !S2) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
-    Plan pl = make_plan(data, E, M, T / M, F, nullptr, E, true, false);
+    Plan pl = make_plan(data, E, M, T / M, F, nullptr, E, true, false, 1);
     if ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
     p.first_n = E;
+    p.nlev = 1;
     p.S1out = S1; p.S2out = S2;
     return launch_cells(pl, p, (cudaStream_t)stream);
 }
 
 size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M) {
     if (check_shape(T, F, E, M)) return 0;
-    const uint32_t cells = (T / M) * F;
-    return workspace_bytes(cells, (E + 15u) / 16u);     // room for the narrowest slabs any plan uses
+    return workspace_bytes(T / M, F, E, 1);
 }
 
-static int frame_impl(const uint8_t* data, uint32_t T,
-                      uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset, uint32_t first_n,
-                      float n_sigma, float sk_mean, int flags, float* SK, uint8_t* mask, uint32_t* S1o,
-                      uint32_t* S2o, void* workspace, size_t workspace_bytes_given, cudaStream_t st) {
-    if (!SK) return SK_ERR_NULL;
-    if (int rc = check_shape(T, F, E, M)) return rc;
-    if (!subset && (first_n == 0 || first_n > E)) return SK_ERR_N;
-    if (mask && (!std::isfinite(n_sigma) || !std::isfinite(sk_mean) || n_sigma < 0)) return SK_ERR_PARAM;
-    if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
-    Plan pl = make_plan(data, E, M, T / M, F, subset, first_n, S1o != nullptr, (flags & SK_FRAME_INPUTS_READY) != 0);
-    if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
-    sk::FrameParams p{};
-    p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = T / M;
-    p.subset = subset; p.first_n = subset ? 0 : first_n;
-    p.n_sigma = n_sigma; p.sk_mean = sk_mean;
-    p.inputs_ready = (flags & SK_FRAME_INPUTS_READY) ? 1u : 0u;
-    p.SK = SK; p.mask = mask; p.S1out = S1o; p.S2out = S2o;
-    if (pl.vec) {
-        const uint32_t cells = p.B * F;
-        const size_t need = workspace_bytes(cells, pl.slabs);
-        if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) || workspace_bytes_given < need)
-            return SK_ERR_WORKSPACE;
-        p.partial = static_cast<double*>(workspace);
-        // counters sit after the largest possible partial array, so their place does not depend
-        // on first_n or on the slab width and a workspace stays clean across calls
-        const uint32_t slabs_max = (E + 15u) / 16u;
-        if (workspace_bytes_given < workspace_bytes(cells, slabs_max)) return SK_ERR_WORKSPACE;
-        p.counter = reinterpret_cast<uint32_t*>(static_cast<double*>(workspace) + (size_t)cells * slabs_max);
-    }
-    return launch_cells(pl, p, st);
+size_t sk_frame_multi_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev) {
+    if (check_shape(T, F, E, M) || nlev < 1 || nlev > (uint32_t)sk::kMaxLevels) return 0;
+    return workspace_bytes(T / M, F, E, nlev);
 }
 
 int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
@@ -274,16 +380,18 @@ int sk_combine(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, u
     sk::FrameParams p{};
     p.T = B * M; p.F = F; p.E = E; p.M = M; p.B = B;
     p.subset = subset; p.first_n = subset ? 0 : first_n;
-    p.SK = SK; p.S1in = S1; p.S2in = S2;
+    p.nlev = 1;
+    p.lev[0].SK = SK; p.S1in = S1; p.S2in = S2;
     const uint32_t cells = B * F;
     const bool vec = E % 16 == 0 &&
                      ((reinterpret_cast<uintptr_t>(S1) | reinterpret_cast<uintptr_t>(S2)) & 15u) == 0;
     if (vec) {
-        const int L = lanes_per_row(E, cells, M, false);
+        // one CTA per cell keeps the cell's per-slab partials in shared memory: widest slabs
+        int L = 16;
+        while (L > 1 && (uint32_t)L > E / 16) L >>= 1;
         p.slabs = (E + 16u * L - 1) / (16u * L);
         p.nunits = cells * p.slabs;
-        const size_t smem = (size_t)p.slabs * sizeof(double);
-        if (smem > 48 * 1024) return SK_ERR_SHAPE;
+        const size_t smem = (size_t)p.slabs * sizeof(double);      // E <= 2^20: at most 32 KiB
         const unsigned block = sk::kWarpsPerCta * 32;
         switch (L) {
             case 16: sk::sk_combine_kernel<16><<<cells, block, smem, st>>>(p); break;
@@ -318,18 +426,21 @@ int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, cons
              uint32_t first_n, float n_sigma, float sk_mean, int flags, float* SK, uint8_t* mask,
              uint32_t* S1_opt, uint32_t* S2_opt, void* workspace, size_t workspace_bytes_given,
              void* stream) {
-    const int zero_flagged = flags & SK_FRAME_ZERO_FLAGGED;
     if (!data || !SK || !mask) return SK_ERR_NULL;
-    cudaStream_t st = (cudaStream_t)stream;
-    int rc = frame_impl(data, T, F, E, M, subset, first_n, n_sigma, sk_mean, flags, SK, mask,
-                        S1_opt, S2_opt, workspace, workspace_bytes_given, st);
-    if (rc != SK_OK || !zero_flagged) return rc;
-    const uint32_t cells = (T / M) * F;
-    const dim3 grid(cells, (M + sk::kExciseRows - 1) / sk::kExciseRows);
-    if (vector_ok(data, E)) sk::sk_excise_kernel<true><<<grid, 256, 0, st>>>(data, mask, F, E, M);
-    else                    sk::sk_excise_kernel<false><<<grid, 256, 0, st>>>(data, mask, F, E, M);
-    ++g_launches;
-    return launch_status();
+    return frame_impl(data, T, F, E, M, 1, subset, first_n, n_sigma, &sk_mean, flags, &SK, &mask, S1_opt,
+                      S2_opt, workspace, workspace_bytes_given, (cudaStream_t)stream);
+}
+
+int sk_frame_multi(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev,
+                   const uint8_t* subset, uint32_t first_n, float n_sigma, const float* h_sk_means, int flags,
+                   float* const* h_SK, uint8_t* const* h_mask, void* workspace, size_t workspace_bytes_given,
+                   void* stream) {
+    if (!data || !h_sk_means || !h_SK || !h_mask) return SK_ERR_NULL;
+    if (nlev < 1 || nlev > (uint32_t)sk::kMaxLevels) return SK_ERR_SHAPE;
+    for (uint32_t l = 0; l < nlev; ++l)
+        if (!h_SK[l] || !h_mask[l]) return SK_ERR_NULL;
+    return frame_impl(data, T, F, E, M, nlev, subset, first_n, n_sigma, h_sk_means, flags, h_SK, h_mask, nullptr,
+                      nullptr, workspace, workspace_bytes_given, (cudaStream_t)stream);
 }
 
 int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
@@ -337,21 +448,30 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
                   uint8_t* h_mask, uint8_t* d_data, float* d_SK, uint8_t* d_mask, void* workspace,
                   size_t workspace_bytes_given, void* stream) {
     if (!h_data || !h_SK || !h_mask || !d_data || !d_SK || !d_mask) return SK_ERR_NULL;
+    // every argument error is reported before the upload is enqueued
     if (int rc = check_shape(T, F, E, M)) return rc;
+    if (int rc = check_frame_args(subset, E, first_n, n_sigma, &sk_mean, 1, true)) return rc;
+    if (vector_ok(d_data, E) && (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) ||
+                                 workspace_bytes_given < workspace_bytes(T / M, F, E, 1)))
+        return SK_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = (size_t)T * F * E, cells = (size_t)(T / M) * F;
     cudaError_t e = cudaMemcpyAsync(d_data, h_data, bytes, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return (int)e;
-    const int zero_flagged = flags & SK_FRAME_ZERO_FLAGGED;
-    const int rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, zero_flagged, d_SK,
-                            d_mask, nullptr, nullptr, workspace, workspace_bytes_given, stream);
-    if (rc != SK_OK) return rc;
-    e = cudaMemcpyAsync(h_SK, d_SK, cells * sizeof(float), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(h_mask, d_mask, cells, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && zero_flagged)
-        e = cudaMemcpyAsync(h_data, d_data, bytes, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    return e == cudaSuccess ? SK_OK : (int)e;
+    const int keep = flags & (SK_FRAME_ZERO_FLAGGED | SK_FRAME_EQ13);
+    int rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, keep, d_SK, d_mask, nullptr,
+                      nullptr, workspace, workspace_bytes_given, stream);
+    if (rc == SK_OK) {
+        e = cudaMemcpyAsync(h_SK, d_SK, cells * sizeof(float), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_mask, d_mask, cells, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && (flags & SK_FRAME_ZERO_FLAGGED))
+            e = cudaMemcpyAsync(h_data, d_data, bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) rc = (int)e;
+    }
+    // the upload has been enqueued: wait for whatever was, also on an error
+    e = cudaStreamSynchronize(st);
+    if (rc == SK_OK && e != cudaSuccess) rc = (int)e;
+    return rc;
 }
 
 int sk_rebin_sums(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
@@ -456,8 +576,13 @@ const char* sk_strerror(int code) {
     }
 }
 
-int sk_version(void) { return 101; }
+int sk_version(void) { return 200; }
 
 unsigned long long sk_launch_count(void) { return g_launches.load(); }
+
+void sk_debug_set_plan(int path, int lanes) {
+    g_force_path.store(path == SK_PLAN_LDG ? SK_PLAN_LDG : SK_PLAN_AUTO);
+    g_force_lanes.store((lanes >= 1 && lanes <= 16 && (lanes & (lanes - 1)) == 0) ? lanes : 0);
+}
 
 }  // extern "C"

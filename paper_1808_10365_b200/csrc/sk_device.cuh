@@ -35,7 +35,7 @@ __device__ __forceinline__ void loads_issued(uint4 (&v)[U]) {
 // ------------------------------------------------------------------------- a1 + a2, packed
 // One 32-bit word holds 4 samples: byte = (re+8)<<4 | (im+8).
 //   hi(w) = (w & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*re   (one LOP3)
-//   lo(w) = ((w<<4) & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*im (SHF + LOP3)
+//   lo(w) = (rotl(w,4) & 0xF0F0F0F0) ^ 0x80808080 : four signed bytes 16*im (SHF + LOP3)
 // Flipping the top bit of the offset nibble turns it into two's complement, and leaving it in
 // the high nibble of its byte sign-extends it for free (scaled by 16).  Nibble 0 -> -128 = 16*(-8).
 // The two masks live in registers (LOP3 takes one immediate only; with both as literals ptxas
@@ -53,144 +53,125 @@ __device__ __forceinline__ uint32_t and_xor(uint32_t a, uint32_t b, uint32_t c) 
     return d;
 }
 __device__ __forceinline__ uint32_t re16(uint32_t w, const UnpackConsts& k) { return and_xor(w, k.f0, k.x80); }
-__device__ __forceinline__ uint32_t im16(uint32_t w, const UnpackConsts& k) { return and_xor(w << 4, k.f0, k.x80); }
-
-// Sample k of the word: C = [16re_k, 16im_k, 16re_k, 16im_k] (one PRMT), then one DP4A gives
-// C.C + c0 = 512 |x_k|^2 + c0  (|x|^2 <= 128, so 512|x|^2 <= 2^16).
-template <int K>
-__device__ __forceinline__ uint32_t power512(uint32_t r16, uint32_t i16, uint32_t c0) {
-    constexpr uint32_t sel = (uint32_t)K | ((4u + K) << 4) | ((uint32_t)K << 8) | ((4u + K) << 12);
-    const uint32_t c = __byte_perm(r16, i16, sel);
-    return (uint32_t)__dp4a((int)c, (int)c, (int)c0);
+// The shift is written as a rotate (SHF.L.W on the ALU pipe; the bits that wrap around land in a low
+// nibble and are masked off): a plain `w << 4` becomes IMAD.SHL on the fmaheavy pipe, which the
+// IDP and the packed FP32 instructions already fill.
+__device__ __forceinline__ uint32_t rotl4(uint32_t w) {
+    uint32_t d;
+    asm("shf.l.wrap.b32 %0, %1, %1, 4;" : "=r"(d) : "r"(w));
+    return d;
 }
+__device__ __forceinline__ uint32_t im16(uint32_t w, const UnpackConsts& k) { return and_xor(rotl4(w), k.f0, k.x80); }
 
 // ------------------------------------------------------------------------------ a3 variants
-// Accumulator for one input.  Two exact strategies with the same interface:
+// Accumulators for TWO adjacent inputs (one 64-bit register pair of state each), three exact
+// strategies with one interface: add2(c0, c1) adds one sample to each input, c = [16re,16im,16re,16im]
+// (pick<K>); read(i, n, S1, S2) returns the sums of input i in {0, 1} after n samples each.
 //
-// AccPlain: S1 += p; S2 += p*p in two 32-bit registers (shift, add, IMAD per sample).
+// AccPlain2: S1 += p; S2 += p*p in 32-bit registers (shift, add, IMAD per sample).  Any n.
 //
-// AccWide : ONE 64-bit multiply-add per sample.  With q = 512 p + 2^31 (the 2^31 comes free as the
+// AccWide2 : ONE 64-bit multiply-add per sample.  With q = 512 p + 2^31 (the 2^31 comes free as the
 //   DP4A addend), q*q = 2^18 p^2 + 2^41 p + 2^62, so a 64-bit accumulator collects
 //   sum p^2 in bits 18..40 and sum p in bits 41..61; the constant n*2^62 (n = samples added) wraps
 //   mod 2^64 and is removed at read-out.  Exact while sum p^2 < 2^23, i.e. n <= 511 samples
-//   (p^2 <= 2^14) — callers flush at most every 256.
-struct AccPlain {
-    uint32_t s1, s2;
-    static constexpr uint32_t kAddend = 0u;
-    __device__ __forceinline__ void reset() { s1 = 0; s2 = 0; }
-    __device__ __forceinline__ void add(uint32_t q) { const uint32_t p = q >> 9; s1 += p; s2 += p * p; }
-    __device__ __forceinline__ void add_c(uint32_t c) { add((uint32_t)__dp4a((int)c, (int)c, 0)); }
-    __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const { S1 = s1; S2 = s2; }
+//   (p^2 <= 2^14).
+//
+// AccChain2: S1 on the IDP addend chain, S2 on the FP32 pipes with Blackwell's packed FP32.
+//   r starts as the bit pattern of the float 2^23 and every IDP adds 512 p to it:
+//   r_k = IDP(C, C, r_{k-1}).  While 512 sum(p) <= 2^23 the float view of r is exactly
+//   2^23 + 512 sum(p), so d = float(r_k) - float(r_{k-1}) = 512 p_k exactly and
+//   s2 = fma(d, d, s2) = 2^18 sum(p^2) exactly (sum p^2 < 2^24).  The two inputs' r sit in one
+//   aligned register pair and their s2 in another, so ONE sub.rn.f32x2 (SASS FADD2) and ONE
+//   fma.rn.f32x2 (SASS FFMA2) serve both: 3 issue slots per sample (PRMT, IDP, half of each packed
+//   op) instead of 4.  S1 = (r - 2^23 pattern) >> 9.
+//   Limit: sum(p) <= 16384, i.e. n <= 128 samples per lane and unit (p <= 128).
+//   Why not AccWide2 everywhere: IMAD.WIDE costs 4 cycles of the half-rate fmaheavy pipe, the
+//   bottleneck of an all-AccWide kernel (ncu: sm__pipe_fmaheavy_cycles_active 78 %).
+struct AccPlain2 {
+    uint32_t s1[2], s2[2];
+    __device__ __forceinline__ void reset() { s1[0] = s1[1] = s2[0] = s2[1] = 0; }
+    __device__ __forceinline__ void add1(int i, uint32_t c) {
+        const uint32_t p = (uint32_t)__dp4a((int)c, (int)c, 0) >> 9;
+        s1[i] += p;
+        s2[i] += p * p;
+    }
+    __device__ __forceinline__ void add2(uint32_t c0, uint32_t c1) { add1(0, c0); add1(1, c1); }
+    __device__ __forceinline__ void read(int i, uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const { S1 = s1[i]; S2 = s2[i]; }
 };
 
-struct AccWide {
-    unsigned long long a;
-    static constexpr uint32_t kAddend = 0x80000000u;
+struct AccWide2 {
+    unsigned long long a[2];
     static constexpr uint32_t kMaxSamples = 511;
-    __device__ __forceinline__ void reset() { a = 0ull; }
-    __device__ __forceinline__ void add(uint32_t q) { a += (unsigned long long)q * q; }
-    __device__ __forceinline__ void add_c(uint32_t c) { add((uint32_t)__dp4a((int)c, (int)c, (int)kAddend)); }
-    __device__ __forceinline__ void read(uint32_t n, uint32_t& S1, uint32_t& S2) const {
-        const unsigned long long v = a - ((unsigned long long)(n & 3u) << 62);
+    __device__ __forceinline__ void reset() { a[0] = a[1] = 0ull; }
+    __device__ __forceinline__ void add1(int i, uint32_t c) {
+        const uint32_t q = (uint32_t)__dp4a((int)c, (int)c, (int)0x80000000u);
+        a[i] += (unsigned long long)q * q;
+    }
+    __device__ __forceinline__ void add2(uint32_t c0, uint32_t c1) { add1(0, c0); add1(1, c1); }
+    __device__ __forceinline__ void read(int i, uint32_t n, uint32_t& S1, uint32_t& S2) const {
+        const unsigned long long v = a[i] - ((unsigned long long)(n & 3u) << 62);
         S1 = (uint32_t)(v >> 41);
         S2 = (uint32_t)((v & ((1ull << 41) - 1ull)) >> 18);
     }
 };
 
-// AccChain: S1 on the IDP addend chain, S2 on the FP32 pipes (which the integer path leaves idle).
-//   r starts as the bit pattern of the float 2^23 and every IDP adds 512 p to it:
-//   r_k = IDP(C, C, r_{k-1}).  While 512 sum(p) <= 2^23 the float view of r is exactly
-//   2^23 + 512 sum(p), so d = float(r_k) - float(r_{k-1}) = 512 p_k exactly (one FADD) and
-//   s2 = fma(d, d, s2) = 2^18 sum(p^2) exactly (sum p^2 < 2^24).  S1 = (r - 2^23 pattern) >> 9.
-//   Limit: sum(p) <= 16384, i.e. n <= 128 samples per lane and unit (p <= 128).
-//   Why: IMAD.WIDE costs 4 cycles of the half-rate fmaheavy pipe, the bottleneck of an all-AccWide
-//   kernel (ncu: sm__pipe_fmaheavy_cycles_active 78 %); FADD/FFMA also run on fmalite.
-struct AccChain {
-    uint32_t r;
-    float s2;
+__device__ __forceinline__ unsigned long long pack2(uint32_t lo, uint32_t hi) {
+    unsigned long long v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "r"(lo), "r"(hi));
+    return v;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, uint32_t& lo, uint32_t& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(v));
+}
+
+struct AccChain2 {
+    uint32_t r0, r1;               // the two IDP chains (float view: 2^23 + 512 sum p)
+    unsigned long long s2;         // two floats: 2^18 sum p^2 of input 0 (low word) and input 1
     static constexpr uint32_t kMagic = 0x4B000000u;
     static constexpr uint32_t kMaxSamples = 128;
-    __device__ __forceinline__ void reset() { r = kMagic; s2 = 0.0f; }
-    __device__ __forceinline__ void add_c(uint32_t c) {
-        const uint32_t r2 = (uint32_t)__dp4a((int)c, (int)c, (int)r);
-#ifndef SK_PROBE_NO_S2                              // experiments only: energy share of the FP32 half
-        const float d = __fsub_rn(__uint_as_float(r2), __uint_as_float(r));
-        s2 = __fmaf_rn(d, d, s2);
-#endif
-        r = r2;
+    __device__ __forceinline__ void reset() { r0 = r1 = kMagic; s2 = 0ull; }
+    __device__ __forceinline__ void add2(uint32_t c0, uint32_t c1) {
+        const uint32_t n0 = (uint32_t)__dp4a((int)c0, (int)c0, (int)r0);
+        const uint32_t n1 = (uint32_t)__dp4a((int)c1, (int)c1, (int)r1);
+        unsigned long long d;
+        asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pack2(n0, n1)), "l"(pack2(r0, r1)));
+        asm("fma.rn.f32x2 %0, %1, %1, %2;" : "=l"(s2) : "l"(d), "l"(s2));
+        r0 = n0;
+        r1 = n1;
     }
-    __device__ __forceinline__ void read(uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const {
-        S1 = (r - kMagic) >> 9;
-        S2 = __float2uint_rn(s2 * (1.0f / 262144.0f));
+    __device__ __forceinline__ void read(int i, uint32_t /*n*/, uint32_t& S1, uint32_t& S2) const {
+        uint32_t lo, hi;
+        unpack2(s2, lo, hi);
+        S1 = ((i ? r1 : r0) - kMagic) >> 9;
+        S2 = __float2uint_rn(__uint_as_float(i ? hi : lo) * (1.0f / 262144.0f));
     }
 };
 
-// [16re_k, 16im_k, 16re_k, 16im_k] of sample K of a word (one PRMT).
+// [16re_k, 16im_k, 16re_k, 16im_k] of sample K of a word (one PRMT); C.C = 512 |x_k|^2 (one IDP.4A).
 template <int K>
 __device__ __forceinline__ uint32_t pick(uint32_t r16, uint32_t i16) {
     constexpr uint32_t sel = (uint32_t)K | ((4u + K) << 4) | ((uint32_t)K << 8) | ((4u + K) << 12);
     return __byte_perm(r16, i16, sel);
 }
 
-// Add the 16 samples of one 128-bit load to 16 accumulators.
-template <class Acc>
-__device__ __forceinline__ void accumulate16(Acc (&acc)[16], const uint4& v, const UnpackConsts& kc) {
+// Add the 16 samples of one 128-bit load to the lane's 16 inputs (8 pair accumulators).
+template <class Acc2>
+__device__ __forceinline__ void accumulate16(Acc2 (&acc)[8], const uint4& v, const UnpackConsts& kc) {
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
-        acc[4 * i + 0].add_c(pick<0>(r, m));
-        acc[4 * i + 1].add_c(pick<1>(r, m));
-        acc[4 * i + 2].add_c(pick<2>(r, m));
-        acc[4 * i + 3].add_c(pick<3>(r, m));
+        acc[2 * i + 0].add2(pick<0>(r, m), pick<1>(r, m));
+        acc[2 * i + 1].add2(pick<2>(r, m), pick<3>(r, m));
     }
 }
 
-// The same with the accumulators split over the pipes: of the 4 inputs of every 32-bit word the
-// first NW use the AccWide accumulators a[], the other 4 - NW the AccChain accumulators b[].
-#ifndef SK_NWIDE
-#define SK_NWIDE 0
-#endif
-constexpr int kNWide = SK_NWIDE;                   // per word; measured on B200: 0 (all AccChain) is fastest
-
-struct AccSplit {
-    AccWide a[4 * kNWide > 0 ? 4 * kNWide : 1];
-    AccChain b[4 * (4 - kNWide) > 0 ? 4 * (4 - kNWide) : 1];
-    __device__ __forceinline__ void reset() {
+// S1, S2 of the lane's 16 inputs after n samples each.
+template <class Acc2>
+__device__ __forceinline__ void read16(const Acc2 (&acc)[8], uint32_t n, uint32_t (&S1)[16], uint32_t (&S2)[16]) {
 #pragma unroll
-        for (int k = 0; k < 4 * kNWide; ++k) a[k].reset();
-#pragma unroll
-        for (int k = 0; k < 4 * (4 - kNWide); ++k) b[k].reset();
-    }
-    template <int I, int K>
-    __device__ __forceinline__ void add_c(uint32_t c) {
-        if (K < kNWide) a[kNWide * I + K].add_c(c);
-        else            b[(4 - kNWide) * I + (K - kNWide)].add_c(c);
-    }
-    template <int I>
-    __device__ __forceinline__ void add_word(uint32_t w, const UnpackConsts& kc) {
-        const uint32_t r = re16(w, kc), m = im16(w, kc);
-        add_c<I, 0>(pick<0>(r, m));
-        add_c<I, 1>(pick<1>(r, m));
-        add_c<I, 2>(pick<2>(r, m));
-        add_c<I, 3>(pick<3>(r, m));
-    }
-    __device__ __forceinline__ void add16(const uint4& v, const UnpackConsts& kc) {
-#ifdef SK_PROBE_MEMORY_ONLY                         // experiments only: what the load path alone sustains
-        b[0].r += v.x ^ v.y ^ v.z ^ v.w;
-        return;
-#endif
-        add_word<0>(v.x, kc);
-        add_word<1>(v.y, kc);
-        add_word<2>(v.z, kc);
-        add_word<3>(v.w, kc);
-    }
-    // sums of input 4*i + k of the lane's 16
-    __device__ __forceinline__ void read(int i, int k, uint32_t n, uint32_t& S1, uint32_t& S2) const {
-        if (k < kNWide) a[kNWide * i + k].read(n, S1, S2);
-        else            b[(4 - kNWide) * i + (k - kNWide)].read(n, S1, S2);
-    }
-};
+    for (int k = 0; k < 16; ++k) acc[k / 2].read(k % 2, n, S1[k], S2[k]);
+}
 
 // Scalar a1-a2 for the fallback kernel.
 __device__ __forceinline__ uint32_t power_scalar(uint8_t byte) {
@@ -233,6 +214,15 @@ __device__ __forceinline__ double eq11_term(double M, double MM, uint32_t S1, ui
 __device__ __forceinline__ float eq14_sk(double S2bar, double M, double N) {
     const double a = __ddiv_rn(__dadd_rn(M, 1.0), __dsub_rn(M, 1.0));
     const double c = __ddiv_rn(S2bar, __dmul_rn(M, N));
+    return __double2float_rn(__dmul_rn(a, __dsub_rn(c, 1.0)));
+}
+
+// Optional estimator: the un-rescaled SK^ = (MN+1)/(MN-1) * (S2bar/(M N) - 1)  (Eq. 13,
+// second line), then float32.
+__device__ __forceinline__ float eq13_sk(double S2bar, double M, double N) {
+    const double mn = __dmul_rn(M, N);
+    const double a = __ddiv_rn(__dadd_rn(mn, 1.0), __dsub_rn(mn, 1.0));
+    const double c = __ddiv_rn(S2bar, mn);
     return __double2float_rn(__dmul_rn(a, __dsub_rn(c, 1.0)));
 }
 

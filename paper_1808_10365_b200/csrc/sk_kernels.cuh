@@ -15,21 +15,34 @@
 
 namespace sk {
 
+constexpr int kMaxLevels = 4;     // integration lengths M, 2M, 4M, 8M from one pass (sk_frame_multi)
+
+// Outputs of one integration length M << l: arrays [B >> l][F]; workspace of that length.
+struct LevelOut {
+    float* SK;                // nullptr at level 0 = power sums only
+    uint8_t* mask;            // or nullptr
+    double* partial;          // workspace: [cells of this length][slabs]
+    uint32_t* counter;        // workspace: [cells of this length], zero on entry, zero on exit
+    float sk_mean;            // flag centre at this length
+};
+
 struct FrameParams {
     const uint8_t* data;      // [T][F][E]
-    uint32_t T, F, E, M, B;
+    uint8_t* excise;          // == data when flagged cells are to be overwritten with 0x88, else nullptr
+    uint32_t T, F, E, M, B;   // M = the shortest integration length, B = T / M
     const uint8_t* subset;    // E bytes or nullptr
     uint32_t first_n;         // used when subset == nullptr
-    float n_sigma, sk_mean;
-    float* SK;                // [B][F] or nullptr (power-sums only)
-    uint8_t* mask;            // [B][F] or nullptr
-    uint32_t* S1out;          // [B][F][E] or nullptr
+    float n_sigma;
+    LevelOut lev[kMaxLevels];
+    uint32_t nlev;            // 1 for every call but sk_frame_multi
+    uint32_t eq13;            // estimator: 0 = Eq. 14 (SK~), 1 = Eq. 13 (un-rescaled SK^)
+    uint32_t* S1out;          // [B][F][E] or nullptr (length M only)
     uint32_t* S2out;
     const uint32_t* S1in;     // combine: read sums instead of data
     const uint32_t* S2in;
-    double* partial;          // workspace: [cells][slabs]
-    uint32_t* counter;        // workspace: [cells], zero on entry, zero on exit
     uint32_t inputs_ready;    // stream kernel: read data before waiting for the previous grid
+    uint32_t chunk;           // stream kernel: rows per accumulator read-out (divides M)
+    uint32_t bpu;             // stream kernel: M-row blocks per unit (a multiple of 1 << (nlev-1))
     uint32_t slabs;           // units per cell that are launched
     uint32_t nunits;          // cells * slabs
 };
@@ -99,14 +112,15 @@ __device__ __forceinline__ int reduce_scatter_rows(uint32_t (&v1)[16], uint32_t 
 // units' subtrees like a binary counter.
 
 // a4 + a5 within a unit: Tree(unit's first input, 16 L), identical on all lanes on return.
+// Md = the integration length the sums v1/v2 cover.
 // v1/v2[0..kOwned) are the sums of inputs e_first ..; `owner` is false for the duplicate lanes
 // when RPW = 32.  Called by both fused kernels and by the combine kernel.
 template <int L>
-__device__ __forceinline__ double unit_partial(const FrameParams& p, bool active, bool owner, uint32_t e_first,
-                                               const uint32_t (&v1)[16], const uint32_t (&v2)[16]) {
+__device__ __forceinline__ double unit_partial(const FrameParams& p, double Md, bool active, bool owner,
+                                               uint32_t e_first, const uint32_t* v1, const uint32_t* v2) {
     constexpr int kOwn = Owned<L>::value;
     constexpr int RPW = 32 / L;
-    const double Md = (double)p.M, MM = __dmul_rn(Md, Md);
+    const double MM = __dmul_rn(Md, Md);
     // which of the lane's inputs are combined: decided once, so that the kOwn divisions below
     // are straight-line code the scheduler can interleave
     uint32_t sel = 0;
@@ -191,12 +205,43 @@ __device__ __forceinline__ double poll_partial(const double* slot) {
     return __longlong_as_double((long long)bits);
 }
 
-// a5 (across units) + a6 + a7 for one cell; whole warp calls, lane 0 writes.  32 units at a time:
-// an aligned group of 32 subtrees is summed with the canonical butterfly, groups are merged.
+// a8: every byte of a flagged cell becomes 0x88 (the encoded 0+0i; "excision").  The
+// cell is rows [row0, row0 + rows) of frequency f, all E inputs.  Called by `nthreads` threads
+// (rank tid) once every unit of the cell has published its partial, i.e. after the cell's last
+// read.  VEC: E % 16 == 0 and data 16-byte aligned.
+template <bool VEC>
+__device__ __forceinline__ void excise_cell(const FrameParams& p, uint32_t row0, uint32_t rows, uint32_t f,
+                                            uint32_t tid, uint32_t nthreads) {
+    const size_t rstride = (size_t)p.F * p.E;
+    uint8_t* base = p.excise + ((size_t)row0 * p.F + f) * p.E;
+    if (VEC) {
+        const uint32_t vec_per_row = p.E / 16;
+        const uint4 z = make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
+        for (uint32_t j = 0; j < rows; ++j) {
+            uint4* row = reinterpret_cast<uint4*>(base + (size_t)j * rstride);
+            for (uint32_t c = tid; c < vec_per_row; c += nthreads) row[c] = z;
+        }
+    } else {
+        for (uint32_t j = 0; j < rows; ++j) {
+            uint8_t* row = base + (size_t)j * rstride;
+            for (uint32_t c = tid; c < p.E; c += nthreads) row[c] = 0x88;
+        }
+    }
+}
+
+// a6: the estimator from S2bar.  Eq. 14 (what CHIME runs) unless the caller asked for Eq. 13.
+__device__ __forceinline__ float estimator(const FrameParams& p, double S2bar, double Md, double Nd) {
+    return p.eq13 ? eq13_sk(S2bar, Md, Nd) : eq14_sk(S2bar, Md, Nd);
+}
+
+// a5 (across units) + a6 + a7 for one cell of integration length M << l; whole warp calls, lane 0
+// writes; returns the flag decision on every lane.  32 units at a time: an aligned group of 32
+// subtrees is summed with the canonical butterfly, groups are merged.
 // POLL: the partials are workspace slots that may still be in flight (fused kernels); otherwise
 // they are plain memory that is already complete (combine kernel: shared memory).
 template <bool POLL>
-__device__ __forceinline__ void finalize_cell(const FrameParams& p, uint32_t cell, int lane, const double* partials) {
+__device__ __forceinline__ uint32_t finalize_cell(const FrameParams& p, int l, uint32_t cell, int lane,
+                                                  const double* partials) {
     const uint32_t N = count_receivers(p, lane);
     auto load = [&](uint32_t s) -> double {
         if (s >= p.slabs) return 0.0;
@@ -216,34 +261,42 @@ __device__ __forceinline__ void finalize_cell(const FrameParams& p, uint32_t cel
         }
         S2bar = tm.total();
     }
+    const double Md = (double)(p.M << l);
+    const float sk = estimator(p, S2bar, Md, (double)N);
+    const uint32_t flagged = flag_decision(sk, p.lev[l].sk_mean, flag_threshold(p.n_sigma, Md, (double)N));
     if (lane == 0) {
-        const double Md = (double)p.M;
-        const float sk = eq14_sk(S2bar, Md, (double)N);
-        p.SK[cell] = sk;
-        if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, (double)N));
+        p.lev[l].SK[cell] = sk;
+        if (p.lev[l].mask) p.lev[l].mask[cell] = (uint8_t)flagged;
     }
+    return p.lev[l].mask ? flagged : 0u;
 }
 
-// Fused kernels: publish the unit's partial; the last unit of the cell to arrive finalizes it.
-__device__ __forceinline__ void publish_and_finalize(const FrameParams& p, uint32_t cell, uint32_t slab,
-                                                     int lane, double part) {
-    double* slots = p.partial + (size_t)cell * p.slabs;
+// Fused kernels: publish the unit's partial of cell (b, f) at length M << l; the last unit of the
+// cell to arrive finalizes it and, if asked to, excises it (every unit has finished reading the
+// cell by then).
+__device__ __forceinline__ void publish_and_finalize(const FrameParams& p, int l, uint32_t b, uint32_t f,
+                                                     uint32_t slab, int lane, double part) {
+    const uint32_t cell = b * p.F + f;
+    double* slots = p.lev[l].partial + (size_t)cell * p.slabs;
     uint32_t last = 0;
     if (lane == 0) {
         store_partial(slots + slab, part);
-        last = (atomicAdd(p.counter + cell, 1u) == p.slabs - 1u);
+        last = (atomicAdd(p.lev[l].counter + cell, 1u) == p.slabs - 1u);
     }
     last = __shfl_sync(0xffffffffu, last, 0);
     if (!last) return;
-    finalize_cell<true>(p, cell, lane, slots);
+    const uint32_t flagged = finalize_cell<true>(p, l, cell, lane, slots);
     __syncwarp();
     // leave the workspace all-zero: partials and counter (header contract)
     for (uint32_t s = lane; s < p.slabs; s += 32) slots[s] = 0.0;
-    if (lane == 0) p.counter[cell] = 0u;
+    if (lane == 0) p.lev[l].counter[cell] = 0u;
+    if (flagged && p.excise) excise_cell<true>(p, b * (p.M << l), p.M << l, f, lane, 32);
 }
 
 // --------------------------------------------------------------------------- fused a1..a7
-template <int L, class Acc>
+// Direct-load fallback of the stream kernel (sk_tma.cuh): the same unit decomposition, 128-bit
+// ld.global.nc loads, one integration length.  Acc2 = AccChain2 / AccWide2 / AccPlain2 by block length.
+template <int L, class Acc2>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, kMinCtasPerSm)
 sk_frame_kernel(const FrameParams p) {
     constexpr int RPW = 32 / L;
@@ -258,11 +311,11 @@ sk_frame_kernel(const FrameParams p) {
 
     uint32_t S1[16], S2[16];
     {
-        Acc acc[16];
+        Acc2 acc[8];
         UnpackConsts kc;
         kc.init();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) acc[k].reset();
+        for (int k = 0; k < 8; ++k) acc[k].reset();
         const size_t rstride = (size_t)p.F * p.E;
         const uint8_t* base = p.data + ((size_t)b * p.M * p.F + f) * p.E + e0;
         uint32_t n = 0;
@@ -288,8 +341,7 @@ sk_frame_kernel(const FrameParams p) {
             }
             n = mine;
         }
-#pragma unroll
-        for (int k = 0; k < 16; ++k) acc[k].read(n, S1[k], S2[k]);
+        read16(acc, n, S1, S2);
     }
     const int base = reduce_scatter_rows<L>(S1, S2, r0);
     constexpr int kOwn = Owned<L>::value;
@@ -309,7 +361,8 @@ sk_frame_kernel(const FrameParams p) {
             for (int i = 0; i < kOwn; ++i) { o1[i] = S1[i]; o2[i] = S2[i]; }
         }
     }
-    if (p.SK) publish_and_finalize(p, cell, slab, lane, unit_partial<L>(p, active, owner, e_first, S1, S2));
+    if (p.lev[0].SK)
+        publish_and_finalize(p, 0, b, f, slab, lane, unit_partial<L>(p, (double)p.M, active, owner, e_first, S1, S2));
 }
 
 // ------------------------------------------------------------------ a4..a6 from stored sums
@@ -344,11 +397,11 @@ sk_combine_kernel(const FrameParams p) {
             S1[i] = (active && owner) ? __ldg(p.S1in + (size_t)cell * p.E + e_first + i) : 0u;
             S2[i] = (active && owner) ? __ldg(p.S2in + (size_t)cell * p.E + e_first + i) : 0u;
         }
-        const double part = unit_partial<L>(p, active, owner, e_first, S1, S2);
+        const double part = unit_partial<L>(p, (double)p.M, active, owner, e_first, S1, S2);
         if (lane == 0) partials[slab] = part;
     }
     __syncthreads();
-    if (warp == 0) finalize_cell<false>(p, cell, lane, partials);
+    if (warp == 0) finalize_cell<false>(p, 0, cell, lane, partials);
 }
 
 // ------------------------------------------------------------- scalar fallback (any E, alignment)
@@ -386,12 +439,12 @@ __global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const Fr
                     p.S2out[(size_t)cell * p.E + e] = s2;
                 }
             }
-            if (p.SK && selected(p, e)) {
+            if (p.lev[0].SK && selected(p, e)) {
                 term = eq11_term(Md, MM, s1, s2);
                 ++nsel;
             }
         }
-        if (!p.SK) continue;
+        if (!p.lev[0].SK) continue;
         red[threadIdx.x] = term;
         __syncthreads();
         for (int o = 1; o < kScalarThreads; o <<= 1) {
@@ -401,19 +454,26 @@ __global__ void __launch_bounds__(kScalarThreads) sk_cell_kernel_scalar(const Fr
         if (threadIdx.x == 0) tm.push(red[0]);
         __syncthreads();
     }
-    if (!p.SK) return;
+    if (!p.lev[0].SK) return;
     cnt[threadIdx.x] = nsel;
     __syncthreads();
     for (int o = kScalarThreads / 2; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) cnt[threadIdx.x] += cnt[threadIdx.x + o];
         __syncthreads();
     }
+    __shared__ uint32_t flagged;
     if (threadIdx.x == 0) {
         const double N = (double)cnt[0];
-        const float sk = eq14_sk(tm.total(), Md, N);
-        p.SK[cell] = sk;
-        if (p.mask) p.mask[cell] = flag_decision(sk, p.sk_mean, flag_threshold(p.n_sigma, Md, N));
+        const float sk = estimator(p, tm.total(), Md, N);
+        p.lev[0].SK[cell] = sk;
+        flagged = 0;
+        if (p.lev[0].mask) {
+            flagged = flag_decision(sk, p.lev[0].sk_mean, flag_threshold(p.n_sigma, Md, N));
+            p.lev[0].mask[cell] = (uint8_t)flagged;
+        }
     }
+    __syncthreads();
+    if (flagged && p.excise) excise_cell<false>(p, b * p.M, p.M, f, threadIdx.x, kScalarThreads);
 }
 
 // ------------------------------------------------------------------------------------- a7
@@ -490,36 +550,19 @@ __global__ void sk_significance_kernel(const float* __restrict__ SK, float* __re
 }
 
 // ------------------------------------------------------------------------------------- a8
-// Excision: every byte of every flagged cell becomes 0x88 (the encoded 0+0i).
-// grid = (cells, row chunks); a CTA whose cell is clean exits at once.
+// Excision as a pass of its own (the fused kernels excise in their finalizer; this one serves
+// sk_frame_multi when it has to take one pass per length): every byte of every flagged cell of
+// length M becomes 0x88.  grid = (cells, row chunks); a CTA whose cell is clean exits at once.
 constexpr int kExciseRows = 32;
 
 template <bool VEC>
 __global__ void __launch_bounds__(256)
-sk_excise_kernel(uint8_t* __restrict__ data, const uint8_t* __restrict__ mask, uint32_t F, uint32_t E,
-                 uint32_t M) {
+sk_excise_kernel(const FrameParams p, const uint8_t* __restrict__ mask, uint32_t M) {
     const uint32_t cell = blockIdx.x;
     if (mask[cell] == 0) return;
-    const uint32_t b = cell / F, f = cell % F;
+    const uint32_t b = cell / p.F, f = cell % p.F;
     const uint32_t j0 = blockIdx.y * kExciseRows;
-    const uint32_t j1 = min(M, j0 + kExciseRows);
-    const size_t rstride = (size_t)F * E;
-    uint8_t* base = data + ((size_t)b * M * F + f) * E;
-    if (VEC) {
-        const uint32_t vec_per_row = E / 16;
-        const uint32_t total = (j1 - j0) * vec_per_row;
-        const uint4 z = make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
-        for (uint32_t i = threadIdx.x; i < total; i += blockDim.x) {
-            const uint32_t j = j0 + i / vec_per_row, c = i % vec_per_row;
-            reinterpret_cast<uint4*>(base + (size_t)j * rstride)[c] = z;
-        }
-    } else {
-        const uint32_t total = (j1 - j0) * E;
-        for (uint32_t i = threadIdx.x; i < total; i += blockDim.x) {
-            const uint32_t j = j0 + i / E, c = i % E;
-            base[(size_t)j * rstride + c] = 0x88;
-        }
-    }
+    excise_cell<VEC>(p, b * M + j0, min(M - j0, (uint32_t)kExciseRows), f, threadIdx.x, 256);
 }
 
 }  // namespace sk

@@ -1,13 +1,26 @@
 // sk_tma.cuh — the fused SK kernel with TMA staging (sm_100a): the hot path.
 //
-// One WARP per unit, one warp per CTA.  A unit is one (cell, slab): M time rows x W = 16*L
-// contiguous inputs.  The warp streams its unit through a private shared-memory ring of kStages
-// tiles; a tile is kTileBytes = R rows x W bytes (R = kTileBytes / W) fetched by ONE 2-D TMA bulk
-// copy (cp.async.bulk.tensor -> SASS UTMALDG) that signals an mbarrier when its bytes have landed.
-// Lane 0 refills a slot as soon as the warp has consumed it, so the bytes in flight per SM are
-// (resident warps) x kStages x kTileBytes, independent of registers, and the lanes only ever read
-// shared memory.  No CTA-wide barrier exists anywhere: warps never wait for one another, and the
-// hardware block scheduler deals units to SMs one warp at a time (even to within one unit).
+// One WARP per unit, one warp per CTA.  A unit is one (row range, frequency, slab): p.bpu
+// consecutive M-row blocks x W = 16*L contiguous inputs.  bpu = 1 (one cell) for the plain
+// sk_frame at M >= 256; a multiple of 2^(NLEV-1), so that a unit holds whole cells of the longest
+// of the NLEV integration lengths asked for; and several short blocks when M < 256, so that the
+// unit's set-up is paid once per 256 rows.  The warp streams its rows through a
+// private shared-memory ring of kStages tiles; a tile is kTileBytes = R rows x W bytes
+// (R = kTileBytes / W) fetched by ONE 2-D TMA bulk copy (cp.async.bulk.tensor -> SASS UTMALDG)
+// that signals an mbarrier when its bytes have landed.  Lane 0 refills a slot as soon as the warp
+// has consumed it, so the bytes in flight per SM are (resident warps) x kStages x kTileBytes,
+// independent of registers, and the lanes only ever read shared memory.  No CTA-wide barrier
+// exists anywhere: warps never wait for one another, and the hardware block scheduler deals units
+// to SMs one warp at a time (even to within one unit).
+//
+// The rows are consumed in chunks of p.chunk rows (a divisor of M, at most 128 rows per lane: the
+// exactness limit of AccChain2).  After each chunk the lane's 16 x (S1, S2) are read out of the
+// packed accumulators, the row groups are reduce-scattered (integers, exact) and, with CHUNKED,
+// added to the running sums of the current M-row block.  When a block is complete its Eq. 11 terms
+// go into the unit's float64 partial of length M; with NLEV > 1 the block's integer sums are also
+// added to the running sums of lengths 2M, 4M, ... ("a variety of integration
+// lengths"), each of which is published when its last block has been added.  The TMA ring never
+// drains between chunks or blocks.
 // The arithmetic, the per-unit float64 partial and the finalisation are those of sk_kernels.cuh.
 #pragma once
 #include <cuda.h>
@@ -16,18 +29,12 @@
 
 namespace sk {
 
-#ifndef SK_TILE_BYTES
-#define SK_TILE_BYTES 4096
-#endif
-#ifndef SK_STAGES
-#define SK_STAGES 2
-#endif
-#ifndef SK_MINCTAS
-#define SK_MINCTAS 24
-#endif
-constexpr int kTileBytes = SK_TILE_BYTES;          // bytes per TMA tile (R rows x W inputs)
-constexpr int kStages = SK_STAGES;                 // tiles in flight per warp
-constexpr int kStreamMinCtas = SK_MINCTAS;         // resident warps per SM the register budget allows
+// 8 KiB tiles x 2 stages x 13 resident warps per SM = 208 KiB in flight per SM.  Measured on B200
+// (config 2, GB/s burst / power-capped): 4 KiB x 2 x 24 warps 4760 / 4160 (80 registers: the paired
+// accumulators spill), 4 KiB x 2 x 20 5930 / 4820, 4 KiB x 3 x 16 6060 / 4970, 8 KiB x 2 x 13 6290 / 5140.
+constexpr int kTileBytes = 8192;                   // bytes per TMA tile (R rows x W inputs)
+constexpr int kStages = 2;                         // tiles in flight per warp
+constexpr int kStreamMinCtas = 13;                 // resident warps per SM (16 KiB + barriers of shared memory each)
 constexpr size_t kStreamSmemBytes = (size_t)kStages * kTileBytes + kStages * 8;
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -60,25 +67,31 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
-template <int L>
-__global__ void __launch_bounds__(32, kStreamMinCtas)
+// Several integration lengths keep 16 more running sums per length in registers: a higher
+// register limit (fewer resident warps), so that nothing spills.
+constexpr int stream_max_regs(int nlev) { return nlev == 1 ? 128 : nlev == 2 ? 200 : 232; }
+
+template <int L, int NLEV, bool CHUNKED>
+__global__ void __maxnreg__(stream_max_regs(NLEV))
 sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) {
     constexpr int RPW = 32 / L;                    // rows covered by one warp-wide 128-bit read
     constexpr int W = 16 * L;                      // slab width in inputs (= bytes)
     constexpr int R = kTileBytes / W;              // rows per tile
     constexpr int NLD = R / RPW;                   // 128-bit reads per lane per tile
+    constexpr int kOwn = Owned<L>::value;          // inputs a lane owns after the reduce-scatter
     static_assert(R % RPW == 0 && NLD >= 1, "tile shape");
+    static_assert(NLEV >= 1 && NLEV <= kMaxLevels, "levels");
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x;
     const uint32_t ring = smem_addr(smem);
     const uint32_t bars = ring + kStages * kTileBytes;
 
-    // grid = (slabs, F, B): no integer division on the way to the first load
-    const uint32_t slab = blockIdx.x, f = blockIdx.y, b = blockIdx.z;
-    const uint32_t cell = b * p.F + f;
-    const uint32_t x0 = f * p.E + slab * W, y0 = b * p.M;
-    const uint32_t full = p.M / R;                 // tiles with all R rows inside the block
-    const uint32_t tiles = (p.M + R - 1) / R;
+    // grid = (slabs, F, B / bpu): no integer division on the way to the first load
+    const uint32_t slab = blockIdx.x, f = blockIdx.y;
+    const uint32_t x0 = f * p.E + slab * W;
+    const uint32_t tpc = p.chunk / R;              // tiles per chunk (the host makes chunks of whole tiles)
+    const uint32_t total = (p.M * p.bpu / p.chunk) * tpc;    // tiles of this unit
+    const uint32_t y0 = blockIdx.z * p.M * p.bpu;
 
     // Programmatic dependent launch: let the next grid on the stream start filling SM slots as
     // they free up; wait for the previous grid before the first read unless the caller promised
@@ -93,7 +106,7 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
-            if ((uint32_t)s < tiles) {
+            if ((uint32_t)s < total) {
                 mbar_expect_tx(bars + 8 * s, kTileBytes);
                 tma_load_tile(ring + s * kTileBytes, &tmap, x0, y0 + s * R, bars + 8 * s);
             }
@@ -101,78 +114,100 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
     }
     __syncwarp();
 
-    const int cl = lane % L, r0 = lane / L;
-    const uint32_t e0 = (slab * L + cl) * 16u;
-    const bool active = e0 < p.E;
-    const uint32_t lane_off = r0 * W + cl * 16;
+    const uint32_t lane_off = (lane / L) * W + (lane % L) * 16;
 
     UnpackConsts kc;
     kc.init();
-    AccSplit acc;
-    acc.reset();
-    uint32_t n = 0, t = 0, parity = 0;
-    uint32_t ynext = y0 + kStages * R;             // first row of the tile the next refill fetches
-    // rounds of kStages full tiles: slot numbers are compile-time constants
-    while (t + kStages <= full) {
+    AccChain2 acc[8];
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) {
-            const uint32_t bar = bars + 8 * s;
-            const uint32_t src = ring + s * kTileBytes + lane_off;
-            mbar_wait(bar, parity);
+    for (int k = 0; k < 8; ++k) acc[k].reset();
+    uint32_t run1[CHUNKED ? kOwn : 1], run2[CHUNKED ? kOwn : 1];          // the current block, chunk by chunk
+    uint32_t up1[NLEV > 1 ? NLEV - 1 : 1][kOwn], up2[NLEV > 1 ? NLEV - 1 : 1][kOwn];   // lengths 2M, 4M, ...
+    if (CHUNKED) {
 #pragma unroll
-            for (int i = 0; i < NLD; ++i) acc.add16(lds128(src + i * RPW * W), kc);
-            __syncwarp();                          // every lane has consumed this slot: refill it
-            if (lane == 0 && t + s + kStages < tiles) {
-                mbar_expect_tx(bar, kTileBytes);
-                tma_load_tile(ring + s * kTileBytes, &tmap, x0, ynext + s * R, bar);
-            }
-        }
-        t += kStages;
-        ynext += kStages * R;
-        parity ^= 1;
-        n += kStages * NLD;
+        for (int i = 0; i < kOwn; ++i) run1[i] = run2[i] = 0;
     }
-    // what is left (fewer than kStages full tiles, then a ragged one) is already on its way
-    for (uint32_t s = 0; t < tiles; ++t, ++s) {
+#pragma unroll
+    for (int l = 0; l < NLEV - 1; ++l)
+#pragma unroll
+        for (int i = 0; i < kOwn; ++i) up1[l][i] = up2[l][i] = 0;
+
+    uint32_t s = 0, parity = 0, tc = 0, cq = 0, blk = 0;
+    for (uint32_t g = 0; g < total; ++g) {
         const uint32_t src = ring + s * kTileBytes + lane_off;
         mbar_wait(bars + 8 * s, parity);
-        const uint32_t rows = min((uint32_t)R, p.M - t * R);
-        for (uint32_t r = r0; r < rows; r += RPW) {
-            acc.add16(lds128(src + (r - r0) * W), kc);
-            ++n;
+#pragma unroll
+        for (int i = 0; i < NLD; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+        __syncwarp();                              // every lane has consumed this slot: refill it
+        if (lane == 0 && g + kStages < total) {
+            mbar_expect_tx(bars + 8 * s, kTileBytes);
+            tma_load_tile(ring + s * kTileBytes, &tmap, x0, y0 + (g + kStages) * R, bars + 8 * s);
         }
-    }
+        if (++s == kStages) { s = 0; parity ^= 1; }
+        if (++tc < tpc) continue;
+        tc = 0;
 
-    if (p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");   // before the first write
-
-    uint32_t S1[16], S2[16];
+        // ---- chunk read-out: integer sums of the lane's 16 inputs, row groups reduce-scattered
+        // (what the tile loop does not need is recomputed here, to keep its registers free)
+        const uint32_t sb = blockIdx.z;
+        const int cl = lane % L, r0 = lane / L;
+        const uint32_t e0 = (slab * L + cl) * 16u;
+        const bool active = e0 < p.E;
+        const bool owner = (RPW <= 16) || (r0 < 16);
+        const uint32_t q = p.M / p.chunk;          // chunks per block
+        uint32_t S1[16], S2[16];
+        read16(acc, 0u, S1, S2);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+        for (int k = 0; k < 8; ++k) acc[k].reset();
+        if (!active) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            acc.read(i, k, n, S1[4 * i + k], S2[4 * i + k]);
-            if (!active) { S1[4 * i + k] = 0; S2[4 * i + k] = 0; }
+            for (int k = 0; k < 16; ++k) { S1[k] = 0; S2[k] = 0; }
         }
-    }
-    const int base = reduce_scatter_rows<L>(S1, S2, r0);
-    constexpr int kOwn = Owned<L>::value;
-    const bool owner = (RPW <= 16) || (r0 < 16);
-    const uint32_t e_first = e0 + base;
-    if (p.S1out && active && owner) {
-        uint32_t* o1 = p.S1out + (size_t)cell * p.E + e_first;
-        uint32_t* o2 = p.S2out + (size_t)cell * p.E + e_first;
-        if (kOwn % 4 == 0) {
+        const int base = reduce_scatter_rows<L>(S1, S2, r0);
+        const uint32_t e_first = e0 + base;
+        if (CHUNKED) {
 #pragma unroll
-            for (int i = 0; i < kOwn / 4; ++i) {
-                reinterpret_cast<uint4*>(o1)[i] = make_uint4(S1[4 * i], S1[4 * i + 1], S1[4 * i + 2], S1[4 * i + 3]);
-                reinterpret_cast<uint4*>(o2)[i] = make_uint4(S2[4 * i], S2[4 * i + 1], S2[4 * i + 2], S2[4 * i + 3]);
+            for (int i = 0; i < kOwn; ++i) { run1[i] += S1[i]; run2[i] += S2[i]; }
+            if (++cq < q) continue;
+            cq = 0;
+#pragma unroll
+            for (int i = 0; i < kOwn; ++i) { S1[i] = run1[i]; S2[i] = run2[i]; run1[i] = run2[i] = 0; }
+        }
+
+        // ---- a block of M rows is complete
+        if (p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");   // before the first write
+        const uint32_t b0 = sb * p.bpu + blk;
+        if (p.S1out && active && owner) {
+            const size_t cell = (size_t)b0 * p.F + f;
+            uint32_t* o1 = p.S1out + cell * p.E + e_first;
+            uint32_t* o2 = p.S2out + cell * p.E + e_first;
+            if (kOwn % 4 == 0) {
+#pragma unroll
+                for (int i = 0; i < kOwn / 4; ++i) {
+                    reinterpret_cast<uint4*>(o1)[i] = make_uint4(S1[4 * i], S1[4 * i + 1], S1[4 * i + 2], S1[4 * i + 3]);
+                    reinterpret_cast<uint4*>(o2)[i] = make_uint4(S2[4 * i], S2[4 * i + 1], S2[4 * i + 2], S2[4 * i + 3]);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kOwn; ++i) { o1[i] = S1[i]; o2[i] = S2[i]; }
             }
-        } else {
+        }
+        if (p.lev[0].SK)
+            publish_and_finalize(p, 0, b0, f, slab, lane,
+                                 unit_partial<L>(p, (double)p.M, active, owner, e_first, S1, S2));
+        ++blk;
 #pragma unroll
-            for (int i = 0; i < kOwn; ++i) { o1[i] = S1[i]; o2[i] = S2[i]; }
+        for (int l = 1; l < NLEV; ++l) {
+#pragma unroll
+            for (int i = 0; i < kOwn; ++i) { up1[l - 1][i] += S1[i]; up2[l - 1][i] += S2[i]; }
+            if ((blk & ((1u << l) - 1u)) == 0u) {  // the last block of a cell of length M << l
+                publish_and_finalize(p, l, (b0 >> l), f, slab, lane,
+                                     unit_partial<L>(p, (double)(p.M << l), active, owner, e_first, up1[l - 1], up2[l - 1]));
+#pragma unroll
+                for (int i = 0; i < kOwn; ++i) up1[l - 1][i] = up2[l - 1][i] = 0;
+            }
         }
     }
-    if (p.SK) publish_and_finalize(p, cell, slab, lane, unit_partial<L>(p, active, owner, e_first, S1, S2));
 }
 
 }  // namespace sk

@@ -61,17 +61,33 @@ SHAPES = [
     (8, 1, 16, 2), (21, 2, 16, 7), (128, 3, 48, 64), (500, 1, 256, 250), (512, 2, 272, 256),
     (768, 1, 2048, 256), (512, 3, 2064, 128), (2048, 1, 512, 1024), (2000, 2, 96, 1000),
     (1024, 5, 32, 512), (66, 1, 4096, 33),
-    # beyond the stream kernel: more than 65535 blocks (grid.z), and blocks too long for its
-    # accumulators (direct-load kernel with AccWide, then AccPlain)
-    (140000, 1, 16, 2), (16384, 1, 32, 8192), (65536, 1, 48, 32768),
+    # long blocks: the stream kernel reads its accumulators out every <= 128 samples per lane
+    # (chunked); the direct-load kernel switches to AccWide2, then AccPlain2
+    (4096, 1, 2048, 2048), (1536, 2, 1024, 768), (16384, 1, 128, 8192), (65536, 1, 64, 32768),
+    # short blocks: several per unit
+    (4096, 2, 2048, 32), (2048, 1, 4096, 64),
+    # beyond the stream kernel: more than 65535 units along time (grid.z), tiny E, and a block
+    # length with no usable divisor (direct-load kernel)
+    (140000, 1, 16, 2), (16384, 1, 32, 8192), (65536, 1, 48, 32768), (2 * 4099, 1, 256, 4099),
 ]
 
 
+@pytest.fixture(autouse=True)
+def automatic_plan(sk):
+    """Every test starts from, and leaves behind, the library's automatic kernel choice."""
+    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+    yield
+    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+
+
+PATHS = {"tma": 0, "ldg": 1}          # SK_PLAN_AUTO (the TMA stream kernel where it applies), SK_PLAN_LDG
+
+
 @pytest.fixture(params=["tma", "ldg"])
-def vector_path(request, monkeypatch):
-    """Both vector kernels (TMA-staged and direct 128-bit loads) must satisfy every parity test;
-    SK_B200_PATH is read by the library on every call."""
-    monkeypatch.setenv("SK_B200_PATH", request.param)
+def vector_path(request, sk):
+    """Both vector kernels (TMA-staged and direct 128-bit loads) must satisfy every parity test:
+    sk_debug_set_plan (the header's test-only entry) forces the direct-load kernel."""
+    sk.sk_debug_set_plan(PATHS[request.param], 0)
     return request.param
 
 
@@ -153,99 +169,125 @@ def test_config1_full_frame(sk, oracle, vector_path):
     assert 0.90 < skv.mean() < 0.93 and skv.std() < 1.2 * np.sqrt(4 / (cfg.M * cfg.E))
 
 
-def _check_sampled_cells(sk, oracle, data, out, M, cells, n_sigma, sk_mean, first_n=None):
-    T, F, E = data.shape
-    for (b, f) in cells:
-        cell = data[b * M:(b + 1) * M, f:f + 1, :].contiguous().cpu()
-        ref = oracle.frame(cell.numpy(), M, n_sigma=n_sigma, sk_mean=sk_mean, first_n=first_n)
-        assert_sk_close(out.SK[b, f].item(), ref["SK"][0, 0])
-        assert out.mask[b, f].item() == ref["mask"][0, 0]
-        if out.S1 is not None:
-            np.testing.assert_array_equal(u32np(out.S1.view(torch.int32)[b, f]), ref["S1"][0, 0])
-            np.testing.assert_array_equal(u32np(out.S2.view(torch.int32)[b, f]), ref["S2"][0, 0])
+def _oracle_null_mean(oracle, cfg, frame=3, blocks=4):
+    """The flag centre the paper's way: SK of an RFI-free simulation with the same
+    per-input sigmas, through the ORACLE."""
+    null = sk_synth.make_frame(cfg.with_(T=blocks * cfg.M, cw_block_inputs=None, cw_freqs=(), burst_fraction=0.0,
+                                         sine_freqs=()), frame=frame)
+    return float(oracle.frame(null.numpy(), cfg.M)["SK"].astype(np.float64).mean())
 
 
-def test_config2_rfi_mix_sampled(sk, oracle):
-    """Config 2 at full size (1 GiB): sampled cells against the oracle one by one, and the
-    injected interference is found."""
+def test_config2_rfi_mix_full(sk, oracle):
+    """Config 2 at full size (1 GiB, 2048 cells): S1, S2, SK and mask of the WHOLE frame against
+    the oracle, and the injected interference is found."""
     cfg = sk_synth.config(2)
     data = sk_synth.make_frame(cfg, device="cuda")
-    null = sk_synth.make_frame(cfg.with_(T=4 * cfg.M, cw_freqs=(), burst_fraction=0.0, sine_freqs=()),
-                               device="cuda", frame=3)
-    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())
+    sk_mean = _oracle_null_mean(oracle, cfg)
     out = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, want_sums=True)
     torch.cuda.synchronize()
-    rng = np.random.default_rng(2)
+    host = data.cpu()
+    ref = oracle.frame(host.numpy(), cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)
+    np.testing.assert_array_equal(u32np(out.S1), ref["S1"])
+    np.testing.assert_array_equal(u32np(out.S2), ref["S2"])
+    assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
+    np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    del out
     inj = sk_synth.rfi_cells(cfg).numpy()
-    cells = [(int(rng.integers(cfg.B)), int(rng.integers(cfg.F))) for _ in range(40)]
-    cells += [(int(b), 13) for b in rng.integers(cfg.B, size=4)] + [(0, 0), (cfg.B - 1, cfg.F - 1)]
-    _check_sampled_cells(sk, oracle, data, out, cfg.M, cells, 5.0, sk_mean)
-    mask = out.mask.cpu().numpy().astype(bool)
+    mask = ref["mask"].astype(bool)
     strong = sk_synth.rfi_cells(cfg, include_sine=False).numpy()
     assert mask[strong].mean() > 0.99               # CW and broadband bursts are all found
     assert mask[~inj].mean() < 0.01
     # the sinusoid lives in 64 of 2048 inputs: in the full-array SK it is a few-sigma effect, but
     # combining only the affected receivers (PAPER.md:171, receiver subsets) finds it in every block
     sub = sk.sk_frame(data, cfg.M, first_n=cfg.sine_inputs, n_sigma=5.0, sk_mean=sk_mean)
-    assert sub.mask[:, 13].float().mean().item() > 0.99
-    # excision of exactly the flagged cells, checked at full size with torch reductions only
-    before = data.clone()
+    rsub = oracle.frame(host.numpy(), cfg.M, first_n=cfg.sine_inputs, n_sigma=5.0, sk_mean=sk_mean)
+    assert_sk_close(sub.SK.cpu().numpy(), rsub["SK"])
+    np.testing.assert_array_equal(sub.mask.cpu().numpy(), rsub["mask"])
+    assert rsub["mask"][:, 13].mean() > 0.99
+    # excision in the same pass: every byte of the frame against the oracle's excised copy
     out_z = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)
     torch.cuda.synchronize()
-    assert torch.equal(out_z.mask, out.mask) and torch.equal(out_z.SK, out.SK)
-    cellview = data.view(cfg.B, cfg.M, cfg.F, cfg.E)
-    m = out.mask.bool()[:, None, :, None]
-    assert bool(((cellview == 0x88) | ~m).all())
-    assert bool(((cellview == before.view_as(cellview)) | m).all())
+    np.testing.assert_array_equal(out_z.mask.cpu().numpy(), ref["mask"])
+    assert_sk_close(out_z.SK.cpu().numpy(), ref["SK"])
+    assert torch.equal(data.cpu(), torch.from_numpy(ref["data"]))
     again = sk.sk_frame(data, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True)   # idempotent
-    assert torch.equal(again.mask, out.mask)
-    assert bool((again.SK[out.mask.bool()] == 0).all())
+    assert torch.equal(again.mask, out_z.mask)
+    assert bool((again.SK[out_z.mask.bool()] == 0).all())
 
 
-def test_config4_streaming_sampled(sk, oracle):
+def _oracle_frame_parallel(oracle, host, M, n_sigma, sk_mean, expect_excised, workers):
+    """oracle.frame (with excision) over disjoint slabs of blocks in `workers` threads (cells are
+    independent; the ctypes call releases the GIL).  The oracle itself is unchanged and
+    single-threaded.  Each slab's excised bytes are compared with `expect_excised` on the spot, so
+    that only SK and mask are kept.  Returns SK, mask, and whether every byte matched."""
+    from concurrent.futures import ThreadPoolExecutor
+    T = host.shape[0]
+    B = T // M
+    per = -(-B // (4 * workers))
+    cuts = [(i * per * M, min(T, (i + 1) * per * M)) for i in range(4 * workers) if i * per * M < T]
+
+    def one(c):
+        r = oracle.frame(host[c[0]:c[1]], M, n_sigma=n_sigma, sk_mean=sk_mean, zero_flagged=True)
+        return r["SK"], r["mask"], bool(np.array_equal(r["data"], expect_excised[c[0]:c[1]]))
+
+    with ThreadPoolExecutor(workers) as ex:
+        parts = list(ex.map(one, cuts))
+    return (np.concatenate([p[0] for p in parts], axis=0), np.concatenate([p[1] for p in parts], axis=0),
+            all(p[2] for p in parts))
+
+
+def test_config4_streaming_full(sk, oracle):
     """Config 4 at full size (8 GiB per frame) the way bench.py --workload cfg4 --zero runs it:
-    frames back to back on one stream with SK_FRAME_INPUTS_READY and in-place excision.  Sampled
-    cells against the oracle one by one; excision checked at full size with torch reductions."""
+    frames back to back on one stream with SK_FRAME_INPUTS_READY and in-place excision.  Frame 1's
+    SK, mask and excised bytes are compared with the oracle over the WHOLE frame (16384 cells;
+    the oracle runs on slabs of blocks in parallel threads)."""
+    import os
     cfg = sk_synth.config(4)
     free = torch.cuda.mem_get_info()[0]
-    if free < 3 * cfg.nbytes + (4 << 30):
-        pytest.skip("needs ~28 GiB of free device memory")
+    if free < 2 * cfg.nbytes + (4 << 30):
+        pytest.skip("needs ~20 GiB of free device memory")
+    sk_mean = _oracle_null_mean(oracle, cfg)
     frames = [sk_synth.make_frame(cfg, device="cuda", frame=i) for i in range(2)]
-    null = sk_synth.make_frame(cfg.with_(T=4 * cfg.M, cw_freqs=(), burst_fraction=0.0, sine_freqs=()),
-                               device="cuda", frame=3)
-    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())
-    before = frames[1].clone()
+    before = frames[1].cpu().numpy()
     ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, frames[0].device, 77)
     outs = [sk.sk_frame(d, cfg.M, n_sigma=5.0, sk_mean=sk_mean, zero_flagged=True, inputs_ready=True, workspace=ws)
             for d in frames]
     torch.cuda.synchronize()
-    rng = np.random.default_rng(4)
-    cells = [(int(rng.integers(cfg.B)), int(rng.integers(cfg.F))) for _ in range(24)] + [(0, 0), (cfg.B - 1, cfg.F - 1)]
-    _check_sampled_cells(sk, oracle, before, outs[1], cfg.M, cells, 5.0, sk_mean)
-    mask = outs[1].mask.bool()
-    strong = sk_synth.rfi_cells(cfg, include_sine=False).cuda()
-    assert mask[strong].float().mean().item() > 0.99
-    assert 0.15 < mask.float().mean().item() < 0.30          # "20% RFI mix"
-    m = mask[:, None, :, None]
-    cellview = frames[1].view(cfg.B, cfg.M, cfg.F, cfg.E)
-    assert bool(((cellview == 0x88) | ~m).all())
-    assert bool(((cellview == before.view_as(cellview)) | m).all())
+    after = frames[1].cpu().numpy()
+    rSK, rmask, bytes_equal = _oracle_frame_parallel(oracle, before, cfg.M, 5.0, sk_mean, after,
+                                                     max(1, min(16, os.cpu_count() or 1)))
+    assert_sk_close(outs[1].SK.cpu().numpy(), rSK)
+    np.testing.assert_array_equal(outs[1].mask.cpu().numpy(), rmask)
+    assert bytes_equal
+    mask = rmask.astype(bool)
+    strong = sk_synth.rfi_cells(cfg, include_sine=False).numpy()
+    assert mask[strong].mean() > 0.99
+    assert 0.15 < mask.mean() < 0.30          # "20% RFI mix"
 
 
-def test_config3_sweep_sampled(sk, oracle):
-    """Config 3 (512 MiB): M x N sweep, sampled cells per point, and the closed-form trend."""
+def test_config3_sweep_full(sk, oracle):
+    """Config 3 (512 MiB): the M x N sweep over the WHOLE frame: the oracle's S1/S2 once per M, its
+    combine / flag per N (first N inputs), against sk_frame at every one of the 25 points; and the
+    closed-form trend of the null moments."""
     cfg = sk_synth.config(3)
     data = sk_synth.make_frame(cfg, device="cuda")
-    rng = np.random.default_rng(3)
+    host = data.cpu().numpy()
     for M in (64, 128, 256, 512, 1024):
+        S1, S2 = oracle.power_sums(host, M)
+        first = True
         for N in (16, 64, 256, 1024, 2048):
-            out = sk.sk_frame(data, M, first_n=N, n_sigma=3.0, sk_mean=0.94)
-            B = cfg.T // M
-            cells = [(int(rng.integers(B)), int(rng.integers(cfg.F))) for _ in range(3)]
-            _check_sampled_cells(sk, oracle, data, out, M, cells, 3.0, 0.94, first_n=N)
-            skv = out.SK.double()
-            assert abs(skv.mean().item() - 0.941) < 0.01 + 4.0 / M         # 4-bit null mean (sigma 2.5)
-            ratio = skv.var().item() / (4.0 / (M * N))
+            out = sk.sk_frame(data, M, first_n=N, n_sigma=3.0, sk_mean=0.94, want_sums=first)
+            rSK = oracle.combine(S1, S2, M, first_n=N)
+            rmask = oracle.flag(rSK, M, N, 3.0, 0.94)
+            assert_sk_close(out.SK.cpu().numpy(), rSK)
+            np.testing.assert_array_equal(out.mask.cpu().numpy(), rmask)
+            if first:
+                np.testing.assert_array_equal(u32np(out.S1), S1)
+                np.testing.assert_array_equal(u32np(out.S2), S2)
+                first = False
+            skv = rSK.astype(np.float64)
+            assert abs(skv.mean() - 0.941) < 0.01 + 4.0 / M                # 4-bit null mean (sigma 2.5)
+            ratio = skv.var(ddof=1) / (4.0 / (M * N))
             assert 0.4 < ratio < 0.9                                       # below first order on 4-bit data
 
 
@@ -270,13 +312,13 @@ def test_unfused_equals_fused(sk, oracle):
         assert torch.equal(SKs.view(torch.int32), fs.SK.view(torch.int32))
 
 
-def test_vector_paths_bit_identical(sk, monkeypatch):
+def test_vector_paths_bit_identical(sk):
     """TMA-staged and direct-load kernels add in the same order: identical bits, ragged M included."""
     for (T, F, E, M) in [(768, 2, 2048, 256), (1000, 3, 528, 250), (2048, 1, 512, 1024), (66, 1, 4096, 33)]:
         data = sk_synth.random_bytes(T, F, E, seed=21).cuda()
         res = {}
         for path in ("tma", "ldg"):
-            monkeypatch.setenv("SK_B200_PATH", path)
+            sk.sk_debug_set_plan(PATHS[path], 0)
             res[path] = sk.sk_frame(data, M, n_sigma=2.0, sk_mean=0.4, want_sums=True)
         torch.cuda.synchronize()
         a, b = res["tma"], res["ldg"]
@@ -286,9 +328,9 @@ def test_vector_paths_bit_identical(sk, monkeypatch):
         assert torch.equal(a.mask, b.mask)
 
 
-def test_sk_independent_of_slab_width_and_kernel(sk, monkeypatch):
+def test_sk_independent_of_slab_width_and_kernel(sk):
     """The sum over inputs follows a canonical tree over the input indices: every slab width
-    (SK_B200_LANES), both vector kernels, the unfused path and the scalar kernel (misaligned
+    (sk_debug_set_plan's lanes), both vector kernels, the unfused path and the scalar kernel (misaligned
     pointer) give the same SK bit for bit, receiver subsets and ragged E included."""
     for (T, F, E, M) in [(512, 2, 2048, 128), (384, 3, 528, 96), (256, 1, 4096 + 48, 64)]:
         data = sk_synth.random_bytes(T, F, E, seed=31)
@@ -302,16 +344,14 @@ def test_sk_independent_of_slab_width_and_kernel(sk, monkeypatch):
         for kw in ({}, {"first_n": E // 3 + 5}, {"subset": sub}):
             ref = sk.sk_frame(mis, M, **kw).SK.clone()          # scalar kernel
             S1, S2 = sk.sk_power_sums(d, M)
-            for lanes in ("16", "8", "4", "2", "1"):
-                monkeypatch.setenv("SK_B200_LANES", lanes)
+            for lanes in (16, 8, 4, 2, 1):
                 for path in ("tma", "ldg"):
-                    monkeypatch.setenv("SK_B200_PATH", path)
+                    sk.sk_debug_set_plan(PATHS[path], lanes)
                     got = sk.sk_frame(d, M, **kw).SK
                     assert torch.equal(got.view(torch.int32), ref.view(torch.int32)), (T, F, E, M, kw.keys(), lanes, path)
-                un = sk.sk_combine(S1, S2, M, **kw)
-                assert torch.equal(un.view(torch.int32), ref.view(torch.int32)), (lanes, "combine")
-            monkeypatch.delenv("SK_B200_LANES")
-            monkeypatch.delenv("SK_B200_PATH")
+            sk.sk_debug_set_plan(0, 0)
+            un = sk.sk_combine(S1, S2, M, **kw)
+            assert torch.equal(un.view(torch.int32), ref.view(torch.int32)), "combine"
 
 
 def test_deterministic_and_workspace_clean(sk, vector_path):
@@ -347,7 +387,7 @@ def test_pipelined_frames_inputs_ready(sk, oracle):
             assert torch.equal(a.S1.view(torch.int32), b.S1.view(torch.int32))
             assert torch.equal(a.S2.view(torch.int32), b.S2.view(torch.int32))
         assert int(ws.abs().sum().item()) == 0
-    # excision between pipelined frames: frame kernel -> excise kernel -> next frame's kernel
+    # excision between pipelined frames (the finalizer of a flagged cell overwrites it)
     work = [d.clone() for d in frames[:4]]
     outs = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, workspace=ws, zero_flagged=True, inputs_ready=True)
             for d in work]
@@ -520,3 +560,83 @@ def test_host_entry_point(sk, oracle):
     assert_sk_close(h_SK.numpy(), ref["SK"])
     np.testing.assert_array_equal(h_mask.numpy(), ref["mask"])
     np.testing.assert_array_equal(host.numpy(), ref["data"])
+
+
+@pytest.mark.parametrize("T,F,E,M,nlev", [(2048, 2, 2048, 256, 4), (1536, 1, 2048, 64, 3), (4096, 3, 528, 128, 2),
+                                          (8192, 1, 1024, 1024, 2), (2000, 2, 272, 250, 4), (640, 1, 37, 20, 3),
+                                          (96, 2, 32, 6, 4)])
+def test_frame_multi_against_oracle(sk, oracle, vector_path, T, F, E, M, nlev):
+    """SURVEY 8(f) NEXT-2, fused ("a variety of integration lengths"): ONE call
+    gives SK and mask at M, 2M, ..., each equal to the oracle's frame at that block length (mask
+    bit-exact, SK 1e-6) and, bit for bit, to a separate sk_frame call at that length."""
+    data = sk_synth.random_bytes(T, F, E, seed=T + nlev)
+    data[: 2 * M, 0, : min(E, 16)] = 0x88
+    d = data.cuda()
+    means = [0.4 + 0.01 * l for l in range(nlev)]
+    got = sk.sk_frame_multi(d, M, nlev, n_sigma=2.0, sk_means=means)
+    torch.cuda.synchronize()
+    for l in range(nlev):
+        ref = oracle.frame(data.numpy(), M << l, n_sigma=2.0, sk_mean=means[l])
+        assert_sk_close(got.SK[l].cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(got.mask[l].cpu().numpy(), ref["mask"])
+        one = sk.sk_frame(d, M << l, n_sigma=2.0, sk_mean=means[l])
+        assert torch.equal(one.SK.view(torch.int32), got.SK[l].view(torch.int32))
+    sub = np.arange(E) % 3 != 1
+    got = sk.sk_frame_multi(d, M, nlev, subset=sub, n_sigma=2.0, sk_means=means)
+    for l in range(nlev):
+        ref = oracle.frame(data.numpy(), M << l, subset=sub, n_sigma=2.0, sk_mean=means[l])
+        assert_sk_close(got.SK[l].cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(got.mask[l].cpu().numpy(), ref["mask"])
+
+
+def test_frame_multi_excision_is_the_union(sk, oracle, vector_path):
+    """sk_frame_multi with excision: every estimate is that of the data BEFORE excision, and a
+    sample is excised when the cell of any length that contains it is flagged."""
+    T, F, E, M, nlev = 4096, 2, 2048, 128, 3
+    data = sk_synth.make_frame(sk_synth.config(2).with_(T=T, F=F, E=E, M=M))
+    d = data.cuda()
+    means = [0.91, 0.912, 0.913]
+    got = sk.sk_frame_multi(d, M, nlev, n_sigma=4.0, sk_means=means, zero_flagged=True)
+    torch.cuda.synchronize()
+    expect = data.numpy().copy()
+    view = expect.reshape(T, F, E)
+    nflag = 0
+    for l in range(nlev):
+        ref = oracle.frame(data.numpy(), M << l, n_sigma=4.0, sk_mean=means[l])
+        assert_sk_close(got.SK[l].cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(got.mask[l].cpu().numpy(), ref["mask"])
+        for b, f in zip(*np.nonzero(ref["mask"])):
+            view[b * (M << l):(b + 1) * (M << l), f, :] = 0x88
+            nflag += 1
+    assert 0 < nflag
+    np.testing.assert_array_equal(d.cpu().numpy(), expect)
+
+
+def test_frame_multi_argument_errors(sk):
+    d = torch.zeros(96, 1, 32, dtype=torch.uint8, device="cuda")
+    with pytest.raises(sk.SKError):
+        sk.sk_frame_multi(d, 32, 2)                        # B = 3 is not a multiple of 2
+    with pytest.raises(sk.SKError):
+        sk.sk_frame_multi(d, 16, 5)                        # more than 4 lengths
+    with pytest.raises(sk.SKError):
+        sk.sk_frame_multi(d, 16, 2, sk_means=[1.0])        # one centre per length
+    big = torch.zeros(2 * 65536, 1, 16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(sk.SKError):
+        sk.sk_frame_multi(big, 65536, 2)                   # 2M would not fit the 32-bit sums
+
+
+@pytest.mark.parametrize("T,F,E,M", [(768, 2, 2048, 256), (300, 1, 100, 100), (512, 3, 272, 64)])
+def test_eq13_mode(sk, oracle, T, F, E, M):
+    """SK_FRAME_EQ13: the un-rescaled multi-receiver estimator, against the
+    oracle's Eq. 13 (float64 -> float32), and its fixed ratio to Eq. 14."""
+    data = sk_synth.random_bytes(T, F, E, seed=13)
+    d = data.cuda()
+    S1, S2 = oracle.power_sums(data.numpy(), M)
+    for kw in ({}, {"first_n": E // 2 + 1}):
+        N = kw.get("first_n", E)
+        got = sk.sk_frame(d, M, eq13=True, **kw).SK.cpu().numpy()
+        ref13 = oracle.eq13_and_s1bar(S1, S2, M, **kw)[0]
+        assert_sk_close(got, ref13.astype(np.float32))
+        sk14 = sk.sk_frame(d, M, **kw).SK.cpu().numpy().astype(np.float64)
+        c = (M * N + 1.0) * (M - 1.0) / ((M * N - 1.0) * (M + 1.0))
+        np.testing.assert_allclose(got, c * sk14, rtol=2e-6, atol=2e-7)
