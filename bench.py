@@ -26,28 +26,30 @@ FALLBACK_HBM_GBS = 6650.0
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=20, help="K: sk_frame calls captured in the CUDA graph")
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="cfg1")
-    ap.add_argument("--no-graph", action="store_true", help="launch step by step instead of one CUDA graph")
     ap.add_argument("--zero", action="store_true", help="excise flagged cells in place (a8)")
-    ap.add_argument("--cooldown", type=float, default=0.5,
-                    help="idle seconds between the warm-up replay and the timed region (see the comment there)")
-    ap.add_argument("--sustained-seconds", type=float, default=1.5,
-                    help="after the timed region, replay the graph back to back for about this long and report "
-                         "the throughput and clocks of the second half as 'sustained' (0 = skip)")
-    ap.add_argument("--sustain", type=int, default=1, metavar="R",
-                    help="replay the K-step graph R times back to back inside the timed region (K*R steps): "
-                         "long enough for the power cap to settle the clocks")
+    ap.add_argument("--seconds", type=float, default=1.0,
+                    help="length of the timed steady-state region: the K-step graph is replayed back to back for "
+                         "about this long inside one CUDA-event pair (after half as long untimed)")
+    ap.add_argument("--burst-seconds", type=float, default=0.02,
+                    help="extra 'burst' object: the same replays for this long after --cooldown seconds of idle "
+                         "(0 = skip); not the headline")
+    ap.add_argument("--cooldown", type=float, default=0.5, help="idle seconds before the burst window")
+    ap.add_argument("--sweep", action="store_true", help="--workload cfg3: time every (M, N) point of config 3")
+    ap.add_argument("--sweep-seconds", type=float, default=0.25, help="timed seconds per sweep point")
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "rebin", "single", "sim", "cm"],
+    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
                     help="A/B timing: ldg = the direct-load kernel instead of the TMA stream kernel (sk_debug_set_plan)")
+    ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 4, 8, 16],
+                    help="A/B timing: force a slab width of 16*lanes inputs (sk_debug_set_plan); 0 = automatic")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -107,7 +109,7 @@ class ClockSampler(threading.Thread):
 
     def __init__(self, index):
         super().__init__(daemon=True)
-        self.samples, self.reasons, self.stop_flag, self.ok = [], set(), False, False
+        self.samples, self.names, self.stop_flag, self.ok = [], {}, False, False
         self.max_mhz = None
         try:
             import pynvml
@@ -124,7 +126,7 @@ class ClockSampler(threading.Thread):
         if not self.ok:
             return
         nv = self.nv
-        names = {
+        self.names = names = {
             nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
             nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
             nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
@@ -144,21 +146,19 @@ class ClockSampler(threading.Thread):
                 except Exception:
                     r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 self.samples.append((t, mhz, r))
-                for bit, nm in names.items():
-                    if r & bit and self.window and self.window[0] <= t <= (self.window[1] or 1e30):
-                        self.reasons.add(nm)
             except Exception:
                 pass
-            time.sleep(0.0005)
+            time.sleep(0.0002)
 
     def summary(self):
-        if not self.ok or not self.samples:
+        """Median SM clock and throttle reasons of the samples INSIDE the window (never of others)."""
+        if not self.ok or not self.window:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
-        lo, hi = self.window if self.window else (0, 1e30)
-        inside = sorted(m for (t, m, _) in self.samples if lo <= t <= (hi or 1e30))
-        allv = sorted(m for (_, m, _) in self.samples)
-        use = inside if inside else allv
-        return {"sm_mhz": use[len(use) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+        lo, hi = self.window
+        inside = [(m, r) for (t, m, r) in list(self.samples) if lo <= t <= (hi or 1e30)]
+        mhz = sorted(m for m, _ in inside)
+        reasons = sorted({nm for _, r in inside for bit, nm in self.names.items() if r & bit})
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": self.max_mhz, "reasons": reasons,
                 "samples": len(inside)}
 
 
@@ -177,7 +177,7 @@ def run_reference(args):
     sub = cfg.with_(T=blocks * cfg.M)
     host = sk_synth.make_frame(sub).numpy()
     steps = max(1, min(args.steps, 20))
-    warm = min(args.warmup, 1)
+    warm = max(0, min(args.warmup, 5))
     for _ in range(warm):
         sk_oracle.frame(host, cfg.M, n_sigma=cfg.n_sigma)
     t0 = time.perf_counter()
@@ -189,7 +189,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M,
+        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "N": cfg.E,
+                   "n_sigma": cfg.n_sigma, "zero_flagged": False,
                    "sample": f"{blocks} of {cfg.B} blocks per step ({host.size} samples)"},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                          "sample": f"{steps} steps x {host.size} samples of {cfg.name}"},
@@ -209,7 +210,7 @@ def run_sim(args):
     cfg = sk_synth.config(1)
     thr = sk_synth.digitiser_thresholds(sk_synth.sigma_per_input(cfg)).cuda()
     bufs = [torch.empty(cfg.T, cfg.F, cfg.E, dtype=torch.uint8, device="cuda") for _ in range(4)]
-    K, W = args.steps if args.steps != 2000 else 20, max(args.warmup, 3)
+    K, W = args.steps, max(args.warmup, 3)
     for i in range(W):
         sk.sk_sim_digitised(cfg.T, cfg.F, cfg.E, thr, 1, i, out=bufs[i % 4])
     torch.cuda.synchronize()
@@ -243,7 +244,7 @@ def run_cm(args):
     import paper_1808_10365_b200 as sk
     torch.cuda.set_device(0)
     D, M, N, amp = 1000, 256, 4096, 0.5
-    K, W = args.steps if args.steps != 2000 else 5, 3
+    K, W = min(args.steps, 5), 3
     for i in range(W):
         sk.sk_sim_common_mode(D, M, N, amp, seed=i)
     torch.cuda.synchronize()
@@ -282,7 +283,7 @@ def run_aux(args):
     n = B * F * E
     fn = (lambda a, b: sk.sk_rebin_sums(a, b, cfg.M, 2)) if args.op == "rebin" else (lambda a, b: sk.sk_single(a, b, cfg.M))
     alg = n * 8 + (n * 8 // 2 if args.op == "rebin" else n * 4)
-    K, W = args.steps if args.steps != 2000 else 50, max(args.warmup, 3)
+    K, W = max(args.steps, 50), max(args.warmup, 3)
     for i in range(W):
         fn(*sums[i % 2])
     torch.cuda.synchronize()
@@ -307,6 +308,158 @@ def run_aux(args):
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
+def null_mean(sk, sk_synth, cfg, dev, M=None):
+    """The flag centre the paper's way: mean SK of an RFI-free simulation with the
+    workload's per-input sigmas (the 4-bit null mean is not 1: App. B)."""
+    M = M or cfg.M
+    null = sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * M), M=M, cw_block_inputs=None, cw_freqs=(),
+                                         burst_fraction=0.0, sine_freqs=()), device=dev, frame=777)
+    return float(sk.sk_frame(null, M).SK.double().mean().item())
+
+
+def timed_replays(torch, graph, stream, seconds, step_s_estimate, steps_per_replay, barrier, sampler=None):
+    """Replay the K-step graph back to back for about `seconds` inside ONE CUDA-event pair on the
+    launching stream.  Returns (ms, replays, clock summary of exactly that window)."""
+    reps = max(1, int(round(seconds / max(step_s_estimate * steps_per_replay, 1e-7))))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_lo = time.perf_counter()
+    if sampler is not None:
+        sampler.window = (t_lo, None)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(reps):
+            graph.replay()
+        e1.record(stream)
+    barrier()
+    t_hi = time.perf_counter()
+    clocks = None
+    if sampler is not None:
+        sampler.window = (t_lo, t_hi)
+        clocks = sampler.summary()
+    return e0.elapsed_time(e1), reps, clocks
+
+
+def run_sweep(args, sk, sk_synth, torch, dev):
+    """--workload cfg3 --sweep: BASELINE.json config 3, throughput at each (M, N): M in {64..1024} x
+    N in {16..2048} (the first N inputs).  Inputs beyond N are never read, so next to the frame's
+    samples/s the line gives the bytes actually moved and the GB/s on those."""
+    cfg = workload("cfg3")
+    nbuf = 2                                              # 2 x 512 MiB > 4 x L2
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=i) for i in range(nbuf)]
+    stream = torch.cuda.Stream(device=dev)
+    peak, peak_src = peaks()
+    K = args.steps
+    points, launches = [], 0
+    for M in (64, 128, 256, 512, 1024):
+        sk_mean = null_mean(sk, sk_synth, cfg, dev, M)
+        B = cfg.T // M
+        for N in (16, 64, 256, 1024, 2048):
+            with torch.cuda.stream(stream):
+                ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, M, dev, stream.cuda_stream)
+                out = sk.sk_frame(bufs[0], M, first_n=N, n_sigma=3.0, sk_mean=sk_mean, workspace=ws, stream=stream)
+            torch.cuda.synchronize()
+
+            def step(i):
+                sk.sk_frame(bufs[i % nbuf], M, first_n=N, n_sigma=3.0, sk_mean=sk_mean, out=out, workspace=ws,
+                            stream=stream, inputs_ready=True)
+            n0 = sk.sk_launch_count()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=stream):
+                for i in range(K):
+                    step(i)
+            launches += sk.sk_launch_count() - n0
+            with torch.cuda.stream(stream):
+                graph.replay()
+            torch.cuda.synchronize()
+            ms, reps, _ = timed_replays(torch, graph, stream, args.sweep_seconds, 1e-4, K, torch.cuda.synchronize)
+            ms, reps, _ = timed_replays(torch, graph, stream, args.sweep_seconds, ms * 1e-3 / (reps * K), K,
+                                        torch.cuda.synchronize)
+            step_s = ms * 1e-3 / (reps * K)
+            lanes, slabs, chunk, bpu = sk.sk_debug_get_plan(cfg.T, cfg.F, cfg.E, M, first_n=N, inputs_ready=True)
+            alg = cfg.T * cfg.F * N + B * cfg.F * 5                                  # N/E of the frame + outputs
+            moved = cfg.T * cfg.F * min(cfg.E, slabs * 16 * lanes) + B * cfg.F * 5   # whole slabs are fetched
+            skv = out.SK.double()
+            points.append({"M": M, "N": N, "us_per_frame": step_s * 1e6,
+                           "frame_samples_per_s": cfg.nbytes / step_s,
+                           "bytes_algorithmic": alg, "gbs_algorithmic": alg / step_s / 1e9,
+                           "bytes_moved": moved, "gbs_on_bytes_moved": moved / step_s / 1e9,
+                           "frac_of_measured_peak": moved / step_s / 1e9 / peak,
+                           "plan": {"slab_bytes": 16 * lanes, "slabs": slabs, "chunk_rows": chunk, "blocks_per_unit": bpu},
+                           "sk_mean": float(skv.mean().item()),
+                           "var_over_first_order": float(skv.var().item()) / (4.0 / (M * N))})
+            del graph
+    full = [p for p in points if p["N"] == cfg.E]
+    line = {"metric": METRIC, "value": sum(p["frame_samples_per_s"] for p in full) / len(full), "unit": UNIT,
+            "n_gpus": 1, "steps": K, "warmup": 1, "ms_per_step": sum(p["us_per_frame"] for p in full) / len(full) * 1e-3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8->u32/f64", "data": "synthetic",
+            "config": {"workload": cfg.name + " (M, N) sweep", "E": cfg.E, "F": cfg.F, "T": cfg.T,
+                       "value_is": "mean over the five N = 2048 points",
+                       "l2": f"rotating over {nbuf} distinct frames of 512 MiB",
+                       "launch": "per point: one CUDA graph of K sk_frame calls replayed for ~%.1f s, "
+                                 "SK_FRAME_INPUTS_READY" % args.sweep_seconds,
+                       "bytes_algorithmic": "T*F*N + 5 B per cell (N/E of the frame)",
+                       "bytes_moved": "T*F*(slabs*slab_bytes) + 5 B per cell: whole slabs are fetched, slabs beyond "
+                                      "first_n are never read",
+                       "sweep": points},
+            "roofline": {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                         "achieved": min(p["gbs_on_bytes_moved"] for p in full),
+                         "frac": min(p["frac_of_measured_peak"] for p in full), "traffic": None,
+                         "note": "the slowest of the five N = 2048 points; per-point figures in config.sweep"},
+            "gpu_launches": int(launches)}
+    print(json.dumps(line))
+
+
+def run_multi(args):
+    """--op multi: sk_frame_multi: SK and mask at M, 2M, 4M, 8M from ONE pass
+    over a config-2 frame, against the single-length sk_frame on the same frames."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = workload("cfg2")
+    nlev = 4
+    nbuf = 4
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=i) for i in range(nbuf)]
+    means = [null_mean(sk, sk_synth, cfg, dev, cfg.M << l) for l in range(nlev)]
+    stream = torch.cuda.Stream(device=dev)
+    K = args.steps
+    with torch.cuda.stream(stream):
+        ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, stream.cuda_stream, nlev)
+        out = sk.sk_frame_multi(bufs[0], cfg.M, nlev, n_sigma=5.0, sk_means=means, workspace=ws, stream=stream)
+    torch.cuda.synchronize()
+    n0 = sk.sk_launch_count()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=stream):
+        for i in range(K):
+            sk.sk_frame_multi(bufs[i % nbuf], cfg.M, nlev, n_sigma=5.0, sk_means=means, out=out, workspace=ws,
+                              stream=stream, inputs_ready=True)
+    launches = sk.sk_launch_count() - n0
+    with torch.cuda.stream(stream):
+        graph.replay()
+    torch.cuda.synchronize()
+    ms, reps, _ = timed_replays(torch, graph, stream, 0.3, 2e-4, K, torch.cuda.synchronize)
+    sampler = ClockSampler(0)
+    sampler.start()
+    ms, reps, clocks = timed_replays(torch, graph, stream, 1.0, ms * 1e-3 / (reps * K), K, torch.cuda.synchronize, sampler)
+    sampler.stop_flag = True
+    step_s = ms * 1e-3 / (reps * K)
+    cells = sum((cfg.B >> l) * cfg.F for l in range(nlev))
+    alg = cfg.nbytes + 5 * cells
+    peak, peak_src = peaks()
+    print(json.dumps({
+        "op": "multi", "metric": METRIC, "value": cfg.nbytes / step_s, "unit": UNIT, "n_gpus": 1, "steps": K,
+        "warmup": 1, "ms_per_step": step_s * 1e3, "higher_is_better": True, "data": "synthetic", "dtype": "u8->u32/f64",
+        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "lengths": [cfg.M << l for l in range(nlev)],
+                   "sk_means": means, "flagged_fraction": [float(m.float().mean().item()) for m in out.mask],
+                   "launch": f"one CUDA graph of K sk_frame_multi calls replayed {reps}x (~1 s), SK_FRAME_INPUTS_READY"},
+        "roofline": {"bound": "hbm", "achieved": alg / step_s / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": alg / step_s / 1e9 / peak, "traffic": stored_traffic("multi"), "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg},
+        "clocks": clocks, "gpu_launches": int(launches)}))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -315,6 +468,8 @@ def main():
         return run_sim(args)
     if args.op == "cm":
         return run_cm(args)
+    if args.op == "multi":
+        return run_multi(args)
     if args.op != "frame":
         return run_aux(args)
 
@@ -334,8 +489,12 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     sk.lib()
-    if args.path == "ldg":
-        sk.sk_debug_set_plan(sk.SK_PLAN_LDG, 0)
+    if args.path == "ldg" or args.lanes:
+        sk.sk_debug_set_plan(sk.SK_PLAN_LDG if args.path == "ldg" else sk.SK_PLAN_AUTO, args.lanes)
+    if args.sweep:
+        if world > 1:
+            raise SystemExit("--sweep is a single-GPU line")
+        return run_sweep(args, sk, sk_synth, torch, dev)
 
     cfg = workload(args.workload)
     K, W = args.steps, max(args.warmup, 3)
@@ -347,15 +506,13 @@ def main():
     nbuf = max(2, min(nbuf, int(free * 0.8) // frame_bytes))
     # every rank draws its own frames (weak scaling: independent frames per GPU, no collective)
     bufs = [sk_synth.make_frame(cfg, device=dev, frame=fid) for fid in frame_ids(rank, nbuf)]
-    null = sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * cfg.M), cw_block_inputs=None, cw_freqs=(),
-                                         burst_fraction=0.0, sine_freqs=()), device=dev, frame=777)
-    sk_mean = float(sk.sk_frame(null, cfg.M).SK.mean().item())     # null mean on 4-bit data
+    sk_mean = null_mean(sk, sk_synth, cfg, dev)
     n_sigma = 5.0
-    outs = [sk.sk_frame(b, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean) for b in bufs[:1]]
-    out = outs[0]
-    ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, 0)
     stream = torch.cuda.Stream(device=dev)
-    pristine = [b.clone() for b in bufs] if args.zero and nbuf * frame_bytes * 2 < free * 0.8 else None
+    with torch.cuda.stream(stream):              # workspace and outputs belong to the timed stream
+        ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, stream.cuda_stream)
+        out = sk.sk_frame(bufs[0], cfg.M, n_sigma=n_sigma, sk_mean=sk_mean, workspace=ws, stream=stream)
+    torch.cuda.synchronize()
 
     # every frame is resident and complete before the timed region starts, and no step writes
     # another step's frame, so the SK_FRAME_INPUTS_READY promise holds (include/sk_b200.h)
@@ -368,78 +525,50 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    with torch.cuda.stream(stream):
-        for i in range(W):
+    for i in range(W):                           # W untimed warm-up steps (with --zero they excise the frames)
+        step(i)
+    if args.zero:
+        for i in range(W, nbuf):
             step(i)
     torch.cuda.synchronize()
     flagged = float(out.mask.float().mean().item())
 
-    graph = None
+    # the graph holds a whole number of K-step passes (>= 200 steps), so that the pipeline bubble at
+    # a graph boundary (the first kernel of a replay does not overlap the last of the previous one)
+    # is amortised the same way whatever K is
+    passes = max(1, -(-200 // K))
+    G = K * passes
     n0 = sk.sk_launch_count()
-    if not args.no_graph:
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph, stream=stream):
-            for i in range(K):
-                step(i)
-        launches = sk.sk_launch_count() - n0
-        with torch.cuda.stream(stream):
-            graph.replay()                      # one untimed replay (graph upload)
-        torch.cuda.synchronize()
-        # The kernel fills 94 % of the issue slots at the full HBM rate and reaches the 1 kW power cap
-        # after ~40 ms of uninterrupted work (sw_power_cap, SM clock 1965 -> ~1520 MHz).  `value` is
-        # the burst figure, like MEASURED_PEAKS.json's hbm_gbs it is compared with: let the power
-        # budget recover after the warm-up; the power-capped figure is reported as `sustained`.
-        time.sleep(args.cooldown)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=stream):
+        for i in range(G):
+            step(i)
+    launches_per_replay = sk.sk_launch_count() - n0
+    with torch.cuda.stream(stream):
+        graph.replay()                           # one untimed replay (graph upload)
+    torch.cuda.synchronize()
 
     sampler = ClockSampler(local)
     sampler.start()
-    e0 = torch.cuda.Event(enable_timing=True)
-    e1 = torch.cuda.Event(enable_timing=True)
-    barrier()
-    t_lo = time.perf_counter()
-    sampler.window = (t_lo, None)
-    with torch.cuda.stream(stream):
-        e0.record(stream)
-        if graph is not None:
-            for _ in range(max(1, args.sustain)):
-                graph.replay()
-        else:
-            n0 = sk.sk_launch_count()
-            for i in range(K):
-                step(i)
-            launches = sk.sk_launch_count() - n0
-        e1.record(stream)
-    barrier()
-    sampler.window = (t_lo, time.perf_counter())
-    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
-    if graph is not None and args.sustain > 1:
-        K *= args.sustain
-        launches *= args.sustain
-
-    # ---- sustained: the same steps back to back until the 1 kW power cap has settled the clocks
-    sustained = None
-    if graph is not None and args.sustained_seconds > 0 and world == 1:
-        reps = max(2, int(args.sustained_seconds / max(ms * 1e-3, 1e-6)) // 2)
-        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        sam2 = ClockSampler(local)
-        sam2.start()
-        with torch.cuda.stream(stream):
-            for _ in range(reps):
-                graph.replay()                  # first half: untimed, lets the clocks settle
-            torch.cuda.synchronize()
-            t_a = time.perf_counter()
-            sam2.window = (t_a, None)
-            s0.record(stream)
-            for _ in range(reps):
-                graph.replay()
-            s1.record(stream)
-        torch.cuda.synchronize()
-        sam2.window = (t_a, time.perf_counter())
-        sam2.stop_flag = True
-        sam2.join(timeout=2)
-        sms = s0.elapsed_time(s1) / (reps * (K // max(1, args.sustain)))
-        sustained = {"value": frame_bytes / (sms * 1e-3), "unit": UNIT, "ms_per_step": sms,
-                     "seconds": s0.elapsed_time(s1) * 1e-3, "clocks": sam2.summary()}
+    # ---- burst: the first ~20 ms after an idle pause.  The kernel draws enough power to reach
+    # the 1 kW cap after ~40 ms of uninterrupted work; before that the SM clock is 1965 MHz.  This is
+    # the counterpart of MEASURED_PEAKS.json's best-of-10 copy; it is NOT the headline.
+    burst = None
+    if args.burst_seconds > 0 and world == 1:
+        ms0, reps0, _ = timed_replays(torch, graph, stream, 0.002, 2e-5 * max(1, frame_bytes >> 26), G, barrier)
+        time.sleep(args.cooldown)
+        bms, breps, bclk = timed_replays(torch, graph, stream, args.burst_seconds, ms0 * 1e-3 / (reps0 * G), G,
+                                         barrier, sampler)
+        burst = {"value": frame_bytes * G * breps / (bms * 1e-3), "unit": UNIT, "ms_per_step": bms / (G * breps),
+                 "seconds": bms * 1e-3, "timed_steps": G * breps, "clocks": bclk,
+                 "protocol": f"{args.cooldown} s idle, then the {G}-step graph replayed {breps}x"}
+    # ---- steady state (the headline): settle for half the window, then time >= `--seconds` of
+    # back-to-back replays inside one CUDA-event pair; the clocks reported are this window's.
+    ms0, reps0, _ = timed_replays(torch, graph, stream, args.seconds / 2, 2e-5 * max(1, frame_bytes >> 26), G, barrier)
+    ms, reps, clocks = timed_replays(torch, graph, stream, args.seconds, ms0 * 1e-3 / (reps0 * G), G, barrier, sampler)
+    ms = max_over_ranks(ms, world, dev)
+    steps_timed = G * reps
+    launches = launches_per_replay * reps
 
     # ---- end to end through the C ABI with host buffers (copies inside the timed region)
     Ke = args.e2e_steps or min(K, 20)
@@ -468,36 +597,44 @@ def main():
             dist.destroy_process_group()
         return
 
-    value = job_value(frame_bytes, world, K, ms)
+    value = job_value(frame_bytes, world, steps_timed, ms)
     cells = cfg.B * cfg.F
     out_bytes = cells * 5
     flagged_bytes = int(flagged * frame_bytes) if args.zero else 0
     alg_bytes = frame_bytes + out_bytes + flagged_bytes          # per launch (1 B/sample read)
     peak, peak_src = peaks()
-    achieved = alg_bytes / (ms * 1e-3 / K) / 1e9
+    achieved = alg_bytes / (ms * 1e-3 / steps_timed) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / steps_timed, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u8->u32/f64", "data": "synthetic",
         "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "N": cfg.E,
                    "n_sigma": n_sigma, "sk_mean": sk_mean, "zero_flagged": bool(args.zero),
                    "frame_bytes": frame_bytes, "flagged_fraction": flagged,
                    "l2": f"rotating over {nbuf} distinct frames ({nbuf * frame_bytes >> 20} MiB > 126 MB L2)",
-                   "launch": ("one CUDA graph of K sk_frame calls" if graph is not None else "K direct sk_frame calls")
+                   "launch": f"one CUDA graph of {passes} x K = {G} sk_frame calls"
                              + ("" if args.serialize else ", SK_FRAME_INPUTS_READY (programmatic dependent launch)"),
+                   "timed_region": f"steady state: the graph replayed {reps}x back to back inside one "
+                                   f"CUDA-event pair ({ms * 1e-3:.2f} s, {steps_timed} steps), after "
+                                   f"{args.seconds / 2:.2f} s of the same to settle the clocks",
+                   "timed_steps": steps_timed, "replays": reps,
                    "parallelism": f"{world} independent replicas (no collective)"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": stored_traffic(cfg.name), "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": stored_traffic(cfg.name + ("_zero" if args.zero else "")),
+                     "peak_source": peak_src,
                      "frac_of_nominal_8000": achieved / 8000.0, "kernel": "sk_stream_kernel",
                      "algorithmic_bytes_per_launch": alg_bytes},
         "e2e": {"value": job_value(frame_bytes, world, Ke, e2e_s * 1e3), "unit": UNIT, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": out_bytes, "steps": Ke, "api": "sk_frame_host (C ABI, pinned host buffers)"},
         "gpu_launches": int(launches),
-        "clocks": sampler.summary(),
+        "clocks": clocks,
     }
-    if sustained is not None:
-        sustained["roofline_frac"] = sustained["value"] * alg_bytes / frame_bytes / 1e9 / peak
-        line["sustained"] = sustained
+    if args.zero:
+        line["config"]["zero_note"] = ("the warm-up excises every frame once; the timed passes flag the same cells "
+                                       "(their SK is 0) and overwrite them again: the traffic of a first pass")
+    if burst is not None:
+        burst["roofline_frac"] = burst["value"] * alg_bytes / frame_bytes / 1e9 / peak
+        line["burst"] = burst
 
     if not args.no_cpu_baseline:
         from oracle import sk_oracle

@@ -190,10 +190,17 @@ unsigned long long sk_launch_count(void);
 /* Tests and A/B timing only: override the kernel choice of the fused path for the whole process.
  * path = SK_PLAN_AUTO (default) or SK_PLAN_LDG (direct-load kernel instead of the TMA stream
  * kernel); lanes = 0 (automatic) or 1, 2, 4, 8, 16: slab width 16*lanes inputs, if not wider than
- * the automatic choice.  Results do not depend on either. */
+ * a row.  Results do not depend on either. */
 #define SK_PLAN_AUTO 0
 #define SK_PLAN_LDG  1
 void sk_debug_set_plan(int path, int lanes);
+
+/* Tests and bench reporting only: the launch plan sk_frame / sk_frame_multi would use for this
+ * shape with a 16-byte-aligned `data` and no subset.  plan4 (HOST, 4 words) = { lanes (slab width
+ * / 16), slabs launched per cell (only those covering first_n), rows per accumulator read-out of
+ * the TMA stream kernel or 0 when the direct-load kernel would run, M-row blocks per unit }. */
+int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags,
+                      uint32_t nlev, uint32_t* plan4);
 
 #ifdef __cplusplus
 }

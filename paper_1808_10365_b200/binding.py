@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
            "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
            "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
-           "sk_launch_count", "sk_debug_set_plan")
+           "sk_launch_count", "sk_debug_set_plan", "sk_debug_get_plan")
 
 # bits of sk_frame's `flags` (include/sk_b200.h)
 SK_FRAME_ZERO_FLAGGED, SK_FRAME_INPUTS_READY, SK_FRAME_EQ13 = 1, 2, 4
@@ -51,6 +51,8 @@ def lib() -> C.CDLL:
     L.sk_frame_multi.argtypes = [vp, u32, u32, u32, u32, u32, vp, u32, f32, vp, i32, vp, vp, vp, sz, vp]
     L.sk_debug_set_plan.argtypes = [i32, i32]
     L.sk_debug_set_plan.restype = None
+    L.sk_debug_get_plan.argtypes = [u32, u32, u32, u32, u32, i32, u32, vp]
+    L.sk_debug_get_plan.restype = i32
     L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
@@ -84,6 +86,15 @@ def sk_debug_set_plan(path: int = SK_PLAN_AUTO, lanes: int = 0) -> None:
     """Tests and A/B timing only (include/sk_b200.h): force the direct-load kernel and / or a
     narrower slab width for the whole process.  (0, 0) restores the automatic choice."""
     lib().sk_debug_set_plan(int(path), int(lanes))
+
+
+def sk_debug_get_plan(T: int, F: int, E: int, M: int, first_n=None, inputs_ready: bool = False, nlev: int = 1):
+    """(lanes, slabs, chunk_rows or 0 for the direct-load kernel, blocks_per_unit) the fused path
+    would use for this shape (aligned data, no subset).  Tests and bench reporting only."""
+    plan = (C.c_uint32 * 4)()
+    _check(lib().sk_debug_get_plan(T, F, E, M, int(first_n or E), SK_FRAME_INPUTS_READY if inputs_ready else 0,
+                                   nlev, C.cast(plan, C.c_void_p)), "sk_debug_get_plan")
+    return tuple(int(x) for x in plan)
 
 
 def _check(rc: int, what: str):

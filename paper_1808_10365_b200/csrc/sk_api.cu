@@ -55,7 +55,7 @@ inline int lanes_per_row(uint32_t E, unsigned long long units_per_slab_column, b
     const unsigned long long want = (unsigned long long)sm_count() * (overlapped ? 8u : 16u);
     while (L > 4 && units_per_slab_column * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
     const int v = g_force_lanes.load(std::memory_order_relaxed);
-    if (v >= 1 && v <= L && (v & (v - 1)) == 0) L = v;
+    if (v >= 1 && (uint32_t)v <= (vecs < 16u ? vecs : 16u) && (v & (v - 1)) == 0) L = v;
     return L;
 }
 
@@ -109,9 +109,11 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
         bpu *= 2u;
     pl.bpu = bpu;
     pl.L = lanes_per_row(E, (unsigned long long)(B / bpu) * F, overlapped);
-    const uint32_t W = 16u * pl.L;
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
+    // a few receivers only: one slab no wider than needed (64 bytes at least), so that the rest of the row is not fetched
+    while (pl.L > 4 && 8u * pl.L >= cover && g_force_lanes.load(std::memory_order_relaxed) == 0) pl.L >>= 1;
+    const uint32_t W = 16u * pl.L;
     pl.slabs = (cover + W - 1) / W;
     const uint32_t RPW = 32u / pl.L;
     const uint32_t iters = (M + RPW - 1) / RPW;
@@ -579,6 +581,21 @@ const char* sk_strerror(int code) {
 int sk_version(void) { return 200; }
 
 unsigned long long sk_launch_count(void) { return g_launches.load(); }
+
+int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags, uint32_t nlev,
+                      uint32_t* plan4) {
+    if (!plan4) return SK_ERR_NULL;
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    if (nlev < 1 || nlev > (uint32_t)sk::kMaxLevels || (T / M) % (1u << (nlev - 1)) != 0) return SK_ERR_SHAPE;
+    if (first_n == 0 || first_n > E) return SK_ERR_N;
+    // an aligned data pointer is assumed (the vector path)
+    const Plan pl = make_plan(nullptr, E, M, T / M, F, nullptr, first_n, false, (flags & SK_FRAME_INPUTS_READY) != 0, nlev);
+    plan4[0] = (uint32_t)pl.L;
+    plan4[1] = pl.slabs;
+    plan4[2] = (pl.vec && stream_wanted(pl)) ? pl.chunk : 0u;
+    plan4[3] = pl.bpu;
+    return SK_OK;
+}
 
 void sk_debug_set_plan(int path, int lanes) {
     g_force_path.store(path == SK_PLAN_LDG ? SK_PLAN_LDG : SK_PLAN_AUTO);

@@ -67,8 +67,11 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
-// Several integration lengths keep 16 more running sums per length in registers: a higher
-// register limit (fewer resident warps), so that nothing spills.
+// 128 registers = 13 resident warps.  Several integration lengths keep 16 more running sums per
+// length and lane (touched once per M-row block) in registers: a higher limit, fewer resident warps.
+// Measured on config 2 with 4 lengths (us per frame; 210 for one length): all in registers,
+// 232-register limit = 8 warps 257; sums in the warp's shared memory, 168 registers = 9 warps 272;
+// 128 registers with the sums spilled to local memory 409.
 constexpr int stream_max_regs(int nlev) { return nlev == 1 ? 128 : nlev == 2 ? 200 : 232; }
 
 template <int L, int NLEV, bool CHUNKED>
