@@ -71,17 +71,42 @@ def peaks():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def stored_traffic(cfg_name):
-    """dram bytes per launch from the committed ncu --set full capture (profiles/), or None."""
+def stored_profile(name):
+    """The row of profiles/roofline_traffic.csv (from the committed ncu --set full captures) for this
+    workload / op, or {}: dram bytes, warp instructions and issue utilisation per launch."""
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == cfg_name:
-                    return int(row["dram_bytes_per_launch"])
+                if row["workload"] == name:
+                    return row
     except Exception:
         pass
-    return None
+    return {}
+
+
+def stored_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed capture, or None."""
+    row = stored_profile(name)
+    return int(row["dram_bytes_per_launch"]) if row else None
+
+
+def issue_roofline(name, samples_per_launch, achieved_samples_per_s):
+    """Roofline object of a kernel bound by instruction issue rather than HBM (the simulators):
+    the ceiling is one warp instruction per cycle and sub-partition (592 x 1.965 GHz) at the
+    instruction count ncu MEASURED for one launch (smsp__inst_executed.sum, committed under
+    profiles/); ncu's own issue utilisation of that launch is given beside it."""
+    row = stored_profile(name)
+    if not row:
+        return None
+    inst = float(row["warp_instructions_per_launch"])
+    per32 = inst * 32.0 / samples_per_launch
+    peak = 592 * 1.965e9 * 32.0 / per32 / 1e9
+    return {"bound": "alu", "achieved": achieved_samples_per_s / 1e9, "unit": "Gsamples/s", "peak": peak,
+            "frac": achieved_samples_per_s / 1e9 / peak, "traffic": int(row["dram_bytes_per_launch"]),
+            "warp_instructions_per_32_samples": per32, "ncu_issue_active_pct": float(row["issue_active_pct"]),
+            "peak_source": "issue slots: 592 sub-partitions x 1.965 GHz / (ncu smsp__inst_executed.sum per sample), "
+                           "profiles/" + row["source"]}
 
 
 def frame_ids(rank, nbuf):
@@ -223,18 +248,12 @@ def run_sim(args):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / K
     mean, var = sk.sk_moments(sk.sk_frame(bufs[0], cfg.M).SK)
-    # issue roofline: the loop body is 225 SASS instructions per row of a receiver pair, i.e. 112 per
-    # sample (Philox4x32-10: 10 rounds x 6; 4 components x 14 compare-adds x 2), one instruction per
-    # cycle per sub-partition: 592 x 32 x 1.965 GHz / 112 = 332 Gsamples/s
-    peak = 592 * 32 * 1.965 / 112
     print(json.dumps({
         "op": "sim", "metric": "simulated_samples_per_s", "value": cfg.nbytes / (ms * 1e-3), "unit": "samples/s",
         "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
         "dtype": "u32->u8", "config": {"workload": cfg.name + " shape, per-input sigma ~ U[1.5,3.5]",
                                        "null_mean": float(mean[0].item()), "null_var": float(var[0].item())},
-        "roofline": {"bound": "alu", "achieved": cfg.nbytes / (ms * 1e-3) / 1e9, "unit": "Gsamples/s",
-                     "peak": peak, "frac": cfg.nbytes / (ms * 1e-3) / 1e9 / peak, "traffic": None,
-                     "peak_source": "issue slots: 112 SASS instructions per sample (DESIGN.md section 9)"},
+        "roofline": issue_roofline("sim", cfg.nbytes, cfg.nbytes / (ms * 1e-3)),
         "gpu_launches": int(sk.sk_launch_count() - n0) }))
 
 
@@ -263,7 +282,8 @@ def run_cm(args):
         "dtype": "f64", "config": {"workload": f"App. A: {D} datasets x n={M} x N={N}, common-mode amplitude {amp}",
                                    "mean": float(mean[0].item()), "var": float(var[0].item()),
                                    "n_eff": 4.0 / (M * float(var[0].item()))},
-        "roofline": None, "gpu_launches": int(sk.sk_launch_count() - n0)}))
+        "roofline": issue_roofline("cm", D * M * N, D * M * N / (ms * 1e-3)),
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
 def run_aux(args):
@@ -303,7 +323,7 @@ def run_aux(args):
         "config": {"workload": f"S1,S2 [{B}][{F}][{E}] uint32 (config 4's size), M={cfg.M}",
                    "l2": "two rotating copies, 256 MiB each"},
         "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                     "frac": alg / (ms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": alg / (ms * 1e-3) / 1e9 / peak, "traffic": stored_traffic(args.op), "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg},
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 

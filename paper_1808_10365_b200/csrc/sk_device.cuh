@@ -202,8 +202,10 @@ __device__ __forceinline__ double div_f64(double n, double y) {
     return __fma_rn(__fma_rn(-y, q, n), r, q);
 }
 
-// term = M^2 S2 / S1^2 in float64 (MM = M*M, exact); numerator and denominator are exact
-// integers below 2^53.  A receiver with S1 == 0 contributes M (header: "A receiver whose S1 is 0").
+// term = M^2 S2 / S1^2 in float64 (MM = M*M, exact).  S1^2 < 2^53 for M <= 65536 only up to S1 < 2^26.5 and
+// M^2 S2 exceeds 2^53 from M ~ 2900 on: each product is then rounded once (round to nearest even), exactly
+// as the oracle's (double)M*M*S2 and (double)S1*S1 are, so the quotient still matches it to one division
+// rounding.  A receiver with S1 == 0 contributes M (header: "A receiver whose S1 is 0").
 __device__ __forceinline__ double eq11_term(double M, double MM, uint32_t S1, uint32_t S2) {
     const double s1 = u32_to_f64(S1), s2 = u32_to_f64(S2);
     const double t = div_f64(__dmul_rn(MM, s2), __dmul_rn(s1, s1));

@@ -1,11 +1,18 @@
 """Seeded synthetic CHIME-shaped inputs for the SK hot path.
 
 This module is shared by the tests, bench.py and smoke(): it produces the byte buffers that BOTH
-the CUDA path and the CPU oracle consume.  It holds none of the method's arithmetic (no decode,
-no power, no S1/S2, no SK): it only draws Gaussian noise, adds the interference signals of
-BASELINE.json's five configs, and quantises to the 4+4-bit offset encoding of PAPER.md:278
-("4+4-bit complex Gaussian data (bounded between -7 and 7)"; bit layout from BASELINE.json:
-high nibble = re + 8, low nibble = im + 8).
+the CUDA path and the CPU oracle consume.  It holds none of the SK arithmetic (no decode, no power,
+no S1/S2, no SK): it only draws Gaussian noise, adds the interference signals of BASELINE.json's
+five configs, and quantises to the 4+4-bit offset encoding of PAPER.md:278 ("4+4-bit complex
+Gaussian data (bounded between -7 and 7)"; bit layout from BASELINE.json: high nibble = re + 8,
+low nibble = im + 8).
+
+One function here IS part of a method the paper describes: `digitiser_thresholds` turns a
+per-receiver sigma into the 14 cumulative thresholds of App. B's round-and-clip digitiser
+(PAPER.md:278).  Both simulators (the oracle's and the device's) take that table as an INPUT, the
+way they take a seed; neither computes it.  It is pinned on its own, against an erf model written
+out in the test (tests/test_oracle_pins.py::test_sim_digitised_layout_and_pmf), so a mistake in it
+cannot hide behind the two sides agreeing with each other.
 
 The paper measured on CHIME / Pathfinder sky data, which is not available here;
 these buffers take its shapes (2048 / 256 inputs, M = 256, 4+4-bit) and stand in for it.

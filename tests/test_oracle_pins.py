@@ -279,6 +279,34 @@ def test_unnormalised_pooling_would_fail(oracle):
     assert abs(pooled.mean() - 1.0) > 0.3 and abs(sk.mean() - 1.0) < 0.01
 
 
+def test_frame_float_layout_at_several_frequencies(oracle):
+    """The float-input entry at F > 1 (its [t][f][e] indexing): integer-valued doubles decoded from
+    random bytes with numpy (not with the oracle) must reproduce the byte entry's S1, S2 exactly
+    (exact integers in float64) and its SK, subset included; and a frequency must see only its own
+    samples (changing f = 1 leaves f = 0 and f = 2 bit-identical)."""
+    rng = np.random.default_rng(21)
+    T, F, E, M = 96, 3, 10, 24
+    data = rng.integers(0, 256, size=(T, F, E), dtype=np.uint8)
+    re = (data >> 4).astype(np.float64) - 8.0
+    im = (data & 15).astype(np.float64) - 8.0
+    S1, S2 = oracle.power_sums(data, M)
+    for kw in ({}, {"first_n": 7}, {"subset": np.arange(E) % 3 != 0}):
+        sk, f1, f2 = oracle.frame_float(re, im, M, **kw)
+        assert np.array_equal(f1, S1.astype(np.float64)) and np.array_equal(f2, S2.astype(np.float64))
+        ref = oracle.combine(S1, S2, M, want64=True, **kw)[1]
+        assert np.array_equal(sk, ref)
+    # hand sums of one cell from the definition (PAPER.md:77 Eq. 7), straight from re/im
+    b, f, e = 2, 1, 4
+    pw = re[b * M:(b + 1) * M, f, e] ** 2 + im[b * M:(b + 1) * M, f, e] ** 2
+    sk, f1, f2 = oracle.frame_float(re, im, M)
+    assert f1[b, f, e] == pw.sum() and f2[b, f, e] == (pw ** 2).sum()
+    re2, im2 = re.copy(), im.copy()
+    re2[:, 1, :] += 1.0
+    sk2 = oracle.frame_float(re2, im2, M)[0]
+    assert np.array_equal(sk2[:, 0], sk[:, 0]) and np.array_equal(sk2[:, 2], sk[:, 2])
+    assert not np.array_equal(sk2[:, 1], sk[:, 1])
+
+
 # ---------------------------------------------------------------------------------------- P9
 def test_skew_and_kurtosis_single_receiver(oracle):
     """N = 1: skew ~ 10/sqrt(M), excess kurtosis ~ 246/M to first order."""
