@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm"],
+    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
@@ -109,6 +109,42 @@ def issue_roofline(name, samples_per_launch, achieved_samples_per_s):
                            "profiles/" + row["source"]}
 
 
+def sm_ceiling(sk, torch, dev, sm_mhz, sm_max_mhz, achieved_samples_per_s, warps=12):
+    """The SM-side ceiling of the hot loop, MEASURED in this run (sk_debug_loop_ceiling: the kernel's
+    a1-a3 loop on a fixed shared-memory tile, no memory traffic, `warps` warps per SM as in the kernel):
+    sub-partition cycles per 32 samples -> samples/s at the SM clock the timed region ran at."""
+    cyc = sk.sk_debug_loop_ceiling(warps, 100, dev)
+    subp = 4 * torch.cuda.get_device_properties(dev).multi_processor_count
+    out = {"subpartition_cycles_per_32_samples": cyc, "warps_per_sm": warps, "subpartitions": subp,
+           "samples_per_s_at_sm_max": subp * 32 * (sm_max_mhz or 1965) * 1e6 / cyc,
+           "what": "sk_debug_loop_ceiling: the stream kernel's tile loop alone (no HBM, TMA, barrier or epilogue)"}
+    if sm_mhz:
+        out["samples_per_s_at_observed_clock"] = subp * 32 * sm_mhz * 1e6 / cyc
+        out["frac_at_observed_clock"] = achieved_samples_per_s / out["samples_per_s_at_observed_clock"]
+    return out
+
+
+def run_ceiling(args):
+    """--op ceiling: the SM-side ceiling of the hot loop for 4..16 warps per SM."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n0 = sk.sk_launch_count()
+    sk.sk_debug_loop_ceiling(12, 20, dev)
+    pts = [{"warps_per_sm": w, "subpartition_cycles_per_32_samples": sk.sk_debug_loop_ceiling(w, 200, dev)}
+           for w in (4, 8, 12, 16)]
+    subp = 4 * torch.cuda.get_device_properties(dev).multi_processor_count
+    best = min(p["subpartition_cycles_per_32_samples"] for p in pts if p["warps_per_sm"] <= 12)
+    print(json.dumps({
+        "op": "ceiling", "metric": "sm_side_ceiling_samples_per_s", "value": subp * 32 * 1.965e9 / best, "unit": "samples/s",
+        "n_gpus": 1, "steps": 1, "warmup": 1, "higher_is_better": True, "data": "synthetic", "dtype": "u8->u32",
+        "config": {"workload": "the stream kernel's tile loop on a fixed shared-memory tile (no HBM traffic)",
+                   "value_is": "sub-partitions x 32 lanes x 1.965 GHz / cycles per 32 samples at 12 warps per SM",
+                   "points": pts},
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
 def frame_ids(rank, nbuf):
     """Frame numbers rank `rank` draws: disjoint between ranks (weak scaling, independent frames)."""
     return [rank * 1000 + i for i in range(nbuf)]
@@ -136,12 +172,17 @@ class ClockSampler(threading.Thread):
         super().__init__(daemon=True)
         self.samples, self.names, self.stop_flag, self.ok = [], {}, False, False
         self.max_mhz = None
+        self.power_limit = None
         try:
             import pynvml
             pynvml.nvmlInit()
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            try:
+                self.power_limit = pynvml.nvmlDeviceGetEnforcedPowerLimit(self.h) / 1000.0
+            except Exception:
+                self.power_limit = None
             self.ok = True
         except Exception:
             self.ok = False
@@ -170,7 +211,11 @@ class ClockSampler(threading.Thread):
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 except Exception:
                     r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                self.samples.append((t, mhz, r))
+                try:
+                    pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                except Exception:
+                    pw = None
+                self.samples.append((t, mhz, r, pw))
             except Exception:
                 pass
             time.sleep(0.0002)
@@ -178,13 +223,16 @@ class ClockSampler(threading.Thread):
     def summary(self):
         """Median SM clock and throttle reasons of the samples INSIDE the window (never of others)."""
         if not self.ok or not self.window:
-            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0, "power_w": None,
+                    "power_limit_w": self.power_limit}
         lo, hi = self.window
-        inside = [(m, r) for (t, m, r) in list(self.samples) if lo <= t <= (hi or 1e30)]
-        mhz = sorted(m for m, _ in inside)
-        reasons = sorted({nm for _, r in inside for bit, nm in self.names.items() if r & bit})
+        inside = [(m, r, pw) for (t, m, r, pw) in list(self.samples) if lo <= t <= (hi or 1e30)]
+        mhz = sorted(m for m, _, _ in inside)
+        watts = sorted(pw for _, _, pw in inside if pw is not None)
+        reasons = sorted({nm for _, r, _ in inside for bit, nm in self.names.items() if r & bit})
         return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": self.max_mhz, "reasons": reasons,
-                "samples": len(inside)}
+                "samples": len(inside), "power_w": watts[len(watts) // 2] if watts else None,
+                "power_limit_w": self.power_limit}
 
 
 def run_reference(args):
@@ -490,6 +538,8 @@ def main():
         return run_cm(args)
     if args.op == "multi":
         return run_multi(args)
+    if args.op == "ceiling":
+        return run_ceiling(args)
     if args.op != "frame":
         return run_aux(args)
 
@@ -649,11 +699,18 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if world == 1:
+        line["roofline"]["sm_ceiling"] = sm_ceiling(sk, torch, dev, (clocks or {}).get("sm_mhz"),
+                                                    (clocks or {}).get("sm_max_mhz"), value)
     if args.zero:
         line["config"]["zero_note"] = ("the warm-up excises every frame once; the timed passes flag the same cells "
                                        "(their SK is 0) and overwrite them again: the traffic of a first pass")
     if burst is not None:
         burst["roofline_frac"] = burst["value"] * alg_bytes / frame_bytes / 1e9 / peak
+        ceil = line["roofline"].get("sm_ceiling")
+        if ceil and (burst["clocks"] or {}).get("sm_mhz"):
+            burst["frac_of_sm_ceiling"] = burst["value"] * ceil["subpartition_cycles_per_32_samples"] / (
+                ceil["subpartitions"] * 32 * burst["clocks"]["sm_mhz"] * 1e6)
         line["burst"] = burst
 
     if not args.no_cpu_baseline:

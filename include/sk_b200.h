@@ -202,6 +202,16 @@ void sk_debug_set_plan(int path, int lanes);
 int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags,
                       uint32_t nlev, uint32_t* plan4);
 
+/* Measurement only (bench.py --op ceiling): the SM-side ceiling of the hot loop.
+ * Runs the stream kernel's tile loop (a1-a3 on 128-bit shared-memory reads) on a fixed shared-memory
+ * tile with no global-memory traffic: one CTA per SM, warps_per_sm (1..16) warps each, `rounds` x 8
+ * tiles of 8 KiB per warp.  sink: device, (SM count) * warps_per_sm * 32 words, written (keeps the
+ * arithmetic alive); cycles: device, one 64-bit word = elapsed SM clocks of CTA 0;
+ * h_samples_per_lane (HOST, may be NULL) = samples every lane has added.  Sub-partition cycles per
+ * 32 samples = cycles / (samples_per_lane * warps_per_sm / 4), warps_per_sm a multiple of 4. */
+int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink, unsigned long long* cycles,
+                          double* h_samples_per_lane, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsk_b200.so")
 SOURCES = ["sk_api.cu"]
-DEPS = ["sk_api.cu", "sk_kernels.cuh", "sk_device.cuh", "sk_tma.cuh", "sk_sim.cuh", os.path.join("..", "..", "include", "sk_b200.h")]
+DEPS = ["sk_api.cu", "sk_kernels.cuh", "sk_device.cuh", "sk_tma.cuh", "sk_sim.cuh", "sk_ceiling.cuh", os.path.join("..", "..", "include", "sk_b200.h")]
 
 
 def nvcc_path() -> str:

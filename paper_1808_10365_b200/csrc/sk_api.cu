@@ -9,6 +9,7 @@
 #include "sk_kernels.cuh"
 #include "sk_tma.cuh"
 #include "sk_sim.cuh"
+#include "sk_ceiling.cuh"
 
 namespace {
 
@@ -595,6 +596,19 @@ int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t f
     plan4[2] = (pl.vec && stream_wanted(pl)) ? pl.chunk : 0u;
     plan4[3] = pl.bpu;
     return SK_OK;
+}
+
+int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink, unsigned long long* cycles,
+                          double* h_samples_per_lane, void* stream) {
+    if (!sink || !cycles) return SK_ERR_NULL;
+    if (warps_per_sm < 1 || warps_per_sm > (uint32_t)sk::kCeilingMaxWarps || rounds == 0) return SK_ERR_SHAPE;
+    const size_t smem = (size_t)warps_per_sm * sk::kTileBytes;
+    cudaFuncSetAttribute(sk::sk_loop_ceiling_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    sk::sk_loop_ceiling_kernel<<<sm_count(), warps_per_sm * 32, smem, (cudaStream_t)stream>>>(sink, cycles, rounds);
+    ++g_launches;
+    // samples every lane of every warp has added: rounds x 8 tiles x 256 samples per lane and tile
+    if (h_samples_per_lane) *h_samples_per_lane = (double)rounds * sk::kCeilingTilesPerReadout * (sk::kTileBytes / 32);
+    return launch_status();
 }
 
 void sk_debug_set_plan(int path, int lanes) {
