@@ -235,6 +235,7 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
         if (stream_wanted(pl)) {
             p.chunk = pl.chunk;
             p.bpu = pl.bpu;
+            p.unit_tiles = p.M * pl.bpu / (sk::kTileBytes / (16u * pl.L));
             const int rc = launch_stream(pl, p, st);
             if (rc != SK_OK) return rc;
         } else if (pl.chain) launch_vec_L<sk::AccChain2>(pl.L, p, st);

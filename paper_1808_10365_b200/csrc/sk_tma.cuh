@@ -93,7 +93,7 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
     const uint32_t slab = blockIdx.x, f = blockIdx.y;
     const uint32_t x0 = f * p.E + slab * W;
     const uint32_t tpc = p.chunk / R;              // tiles per chunk (the host makes chunks of whole tiles)
-    const uint32_t total = (p.M * p.bpu / p.chunk) * tpc;    // tiles of this unit
+    const uint32_t total = p.unit_tiles;           // tiles of this unit: M * bpu / R (from the host: no division here)
     const uint32_t y0 = blockIdx.z * p.M * p.bpu;
 
     // Programmatic dependent launch: let the next grid on the stream start filling SM slots as
@@ -162,9 +162,11 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
         read16(acc, 0u, S1, S2);
 #pragma unroll
         for (int k = 0; k < 8; ++k) acc[k].reset();
-        if (!active) {
+        if (p.E % W != 0u) {                       // a ragged last slab (warp-uniform test): its lanes beyond E add nothing
+            if (!active) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) { S1[k] = 0; S2[k] = 0; }
+                for (int k = 0; k < 16; ++k) { S1[k] = 0; S2[k] = 0; }
+            }
         }
         const int base = reduce_scatter_rows<L>(S1, S2, r0);
         const uint32_t e_first = e0 + base;
