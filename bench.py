@@ -134,6 +134,7 @@ def run_ceiling(args):
     sk.sk_debug_loop_ceiling(12, 20, dev)
     pts = [{"warps_per_sm": w, "subpartition_cycles_per_32_samples": sk.sk_debug_loop_ceiling(w, 200, dev)}
            for w in (4, 8, 12, 16)]
+    pipes = {name: sk.sk_debug_pipe_rate(m, 16, dev) for m, name in enumerate(sk.PIPE_MODES)}
     subp = 4 * torch.cuda.get_device_properties(dev).multi_processor_count
     best = min(p["subpartition_cycles_per_32_samples"] for p in pts if p["warps_per_sm"] <= 12)
     print(json.dumps({
@@ -141,7 +142,9 @@ def run_ceiling(args):
         "n_gpus": 1, "steps": 1, "warmup": 1, "higher_is_better": True, "data": "synthetic", "dtype": "u8->u32",
         "config": {"workload": "the stream kernel's tile loop on a fixed shared-memory tile (no HBM traffic)",
                    "value_is": "sub-partitions x 32 lanes x 1.965 GHz / cycles per 32 samples at 12 warps per SM",
-                   "points": pts},
+                   "points": pts,
+                   "subpartition_cycles_per_warp_instruction": pipes,
+                   "pipes_note": "16 warps per SM, 8 independent chains per lane; pairs count two instructions"},
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 

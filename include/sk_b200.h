@@ -212,6 +212,16 @@ int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t f
 int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink, unsigned long long* cycles,
                           double* h_samples_per_lane, void* stream);
 
+/* Measurement only (bench.py --op ceiling): issue rate of the hot loop's instructions, alone and in
+ * pairs, 8 independent chains per lane.  mode: 0 FFMA, 1 FFMA2 (fma.rn.f32x2), 2 FADD2 (sub.rn.f32x2),
+ * 3 IDP.4A (dp4a), 4 PRMT, 5 IDP + FFMA2, 6 IDP + FFMA, 7 PRMT + FFMA2, 8 IDP + PRMT.  io: device,
+ * 2048 + (SM count) * warps_per_sm * 32 words (the first 2048 are read as operands, the rest written);
+ * cycles: device, elapsed SM clocks of CTA 0; h_instructions_per_warp (HOST, may be NULL) = warp
+ * instructions every warp issued.  Sub-partition cycles per instruction = cycles / (instructions *
+ * warps_per_sm / 4). */
+int sk_debug_pipe_rate(int mode, uint32_t warps_per_sm, uint32_t* io, unsigned long long* cycles,
+                       double* h_instructions_per_warp, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
            "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
            "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
-           "sk_launch_count", "sk_debug_set_plan", "sk_debug_get_plan", "sk_debug_loop_ceiling")
+           "sk_launch_count", "sk_debug_set_plan", "sk_debug_get_plan", "sk_debug_loop_ceiling", "sk_debug_pipe_rate")
 
 # bits of sk_frame's `flags` (include/sk_b200.h)
 SK_FRAME_ZERO_FLAGGED, SK_FRAME_INPUTS_READY, SK_FRAME_EQ13 = 1, 2, 4
@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
     L.sk_debug_get_plan.restype = i32
     L.sk_debug_loop_ceiling.argtypes = [u32, u32, vp, vp, vp, vp]
     L.sk_debug_loop_ceiling.restype = i32
+    L.sk_debug_pipe_rate.argtypes = [i32, u32, vp, vp, vp, vp]
+    L.sk_debug_pipe_rate.restype = i32
     L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
@@ -113,6 +115,24 @@ def sk_debug_loop_ceiling(warps_per_sm: int = 12, rounds: int = 200, device="cud
                                        C.cast(C.pointer(spl), C.c_void_p), _cur()), "sk_debug_loop_ceiling")
     torch.cuda.synchronize(dev)
     return float(cycles.item()) / (spl.value * warps_per_sm / 4.0)
+
+
+PIPE_MODES = ("FFMA", "FFMA2", "FADD2", "IDP.4A", "PRMT", "IDP+FFMA2", "IDP+FFMA", "PRMT+FFMA2", "IDP+PRMT")
+
+
+def sk_debug_pipe_rate(mode: int, warps_per_sm: int = 16, device="cuda") -> float:
+    """Measurement only (include/sk_b200.h): sub-partition cycles per warp instruction of PIPE_MODES[mode]."""
+    dev = torch.device(device)
+    if dev.type != "cuda":
+        raise SKError("sk_debug_pipe_rate needs a CUDA device")
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    io = torch.full((2048 + sms * warps_per_sm * 32,), 0x3F800011, dtype=torch.int32, device=dev)
+    cycles = torch.zeros(1, dtype=torch.int64, device=dev)
+    n = C.c_double(0.0)
+    _check(lib().sk_debug_pipe_rate(mode, warps_per_sm, io.data_ptr(), cycles.data_ptr(),
+                                    C.cast(C.pointer(n), C.c_void_p), _cur()), "sk_debug_pipe_rate")
+    torch.cuda.synchronize(dev)
+    return float(cycles.item()) / (n.value * warps_per_sm / 4.0)
 
 
 def _check(rc: int, what: str):

@@ -612,6 +612,29 @@ int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink
     return launch_status();
 }
 
+int sk_debug_pipe_rate(int mode, uint32_t warps_per_sm, uint32_t* io, unsigned long long* cycles,
+                       double* h_instructions_per_warp, void* stream) {
+    if (!io || !cycles) return SK_ERR_NULL;
+    if (mode < 0 || mode >= sk::kPipeModes || warps_per_sm < 1 || warps_per_sm > (uint32_t)sk::kCeilingMaxWarps)
+        return SK_ERR_SHAPE;
+    const unsigned grid = (unsigned)sm_count(), block = warps_per_sm * 32;
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (mode) {
+        case 0: sk::sk_pipe_rate_kernel<0><<<grid, block, 0, st>>>(io, cycles); break;
+        case 1: sk::sk_pipe_rate_kernel<1><<<grid, block, 0, st>>>(io, cycles); break;
+        case 2: sk::sk_pipe_rate_kernel<2><<<grid, block, 0, st>>>(io, cycles); break;
+        case 3: sk::sk_pipe_rate_kernel<3><<<grid, block, 0, st>>>(io, cycles); break;
+        case 4: sk::sk_pipe_rate_kernel<4><<<grid, block, 0, st>>>(io, cycles); break;
+        case 5: sk::sk_pipe_rate_kernel<5><<<grid, block, 0, st>>>(io, cycles); break;
+        case 6: sk::sk_pipe_rate_kernel<6><<<grid, block, 0, st>>>(io, cycles); break;
+        case 7: sk::sk_pipe_rate_kernel<7><<<grid, block, 0, st>>>(io, cycles); break;
+        default: sk::sk_pipe_rate_kernel<8><<<grid, block, 0, st>>>(io, cycles); break;
+    }
+    ++g_launches;
+    if (h_instructions_per_warp) *h_instructions_per_warp = (double)sk::kPipeIters * 8 * (mode >= 5 ? 2 : 1);
+    return launch_status();
+}
+
 void sk_debug_set_plan(int path, int lanes) {
     g_force_path.store(path == SK_PLAN_LDG ? SK_PLAN_LDG : SK_PLAN_AUTO);
     g_force_lanes.store((lanes >= 1 && lanes <= 16 && (lanes & (lanes - 1)) == 0) ? lanes : 0);

@@ -49,4 +49,51 @@ sk_loop_ceiling_kernel(uint32_t* __restrict__ sink, unsigned long long* __restri
     if (blockIdx.x == 0 && threadIdx.x == 0) *cycles = (unsigned long long)(t1 - t0);
 }
 
+// Issue rate of the loop's instructions, alone and in pairs (the pipe model of DESIGN.md section 6.3):
+// 8 independent chains per lane, 2048 x 8 instructions (or pairs), operands from memory so that nothing
+// folds.  mode: 0 FFMA, 1 FFMA2, 2 FADD2, 3 IDP.4A, 4 PRMT, 5 IDP + FFMA2, 6 IDP + FFMA, 7 PRMT + FFMA2,
+// 8 IDP + PRMT.  *cycles = elapsed SM clocks of CTA 0.
+constexpr int kPipeModes = 9;
+constexpr int kPipeIters = 2048;
+
+template <int MODE>
+__global__ void __launch_bounds__(kCeilingMaxWarps * 32)
+sk_pipe_rate_kernel(uint32_t* __restrict__ io, unsigned long long* __restrict__ cycles) {
+    uint32_t a[8], b[8];
+    unsigned long long p[8], q[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        a[i] = io[i * 32 + (threadIdx.x & 31)];
+        b[i] = io[256 + i * 32 + (threadIdx.x & 31)];
+        p[i] = pack2(io[512 + i * 32 + (threadIdx.x & 31)], io[768 + i * 32 + (threadIdx.x & 31)]);
+        q[i] = pack2(io[1024 + i * 32 + (threadIdx.x & 31)], io[1280 + i * 32 + (threadIdx.x & 31)]);
+    }
+    __syncthreads();
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < kPipeIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (MODE == 3 || MODE == 5 || MODE == 6 || MODE == 8) asm volatile("dp4a.s32.s32 %0, %1, %1, %0;" : "+r"(a[i]) : "r"(b[i]));
+            if (MODE == 4 || MODE == 7) asm volatile("prmt.b32 %0, %0, %1, 0x5140;" : "+r"(a[i]) : "r"(b[i]));
+            if (MODE == 8) asm volatile("prmt.b32 %0, %0, %1, 0x5140;" : "+r"(b[i]) : "r"(a[(i + 3) & 7]));
+            if (MODE == 0) asm volatile("fma.rn.f32 %0, %1, %1, %0;" : "+r"(a[i]) : "r"(b[i]));
+            if (MODE == 6) asm volatile("fma.rn.f32 %0, %1, %1, %0;" : "+r"(b[i]) : "r"(a[i]));
+            if (MODE == 1 || MODE == 5 || MODE == 7) asm volatile("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(p[i]) : "l"(q[i]));
+            if (MODE == 2) asm volatile("sub.rn.f32x2 %0, %1, %0;" : "+l"(p[i]) : "l"(q[i]));
+        }
+    }
+    __syncthreads();
+    const long long t1 = clock64();
+    uint32_t x = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        uint32_t lo, hi;
+        unpack2(p[i], lo, hi);
+        x ^= a[i] ^ b[i] ^ lo ^ hi;
+    }
+    io[2048 + blockIdx.x * blockDim.x + threadIdx.x] = x;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *cycles = (unsigned long long)(t1 - t0);
+}
+
 }  // namespace sk
