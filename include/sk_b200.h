@@ -30,7 +30,8 @@
  *     SK = NaN and mask = 1 for every cell.
  *   - A receiver whose S1 is 0 contributes the term M (its own SK^_i taken as 0), so an
  *     all-0x88 cell gives SK = 0 exactly and re-running on excised data is NaN-free.
- *   - Limits: 2 <= M <= 65536, T % M == 0, T, F, E >= 1, T*F*E < 2^40.
+ *   - Limits: 2 <= M <= 65536, T % M == 0, T, F, E >= 1, T*F*E < 2^40, E <= 2^20, (T/M)*F < 2^31
+ *     (anything beyond returns SK_ERR_SHAPE or SK_ERR_M).
  *     Any E and any alignment is accepted; E % 16 == 0 with a 16-byte-aligned `data` takes the
  *     vector kernels, everything else a slower scalar kernel with identical results.
  *   - Floating point: per-input terms and the sum over inputs are float64 in a fixed order

@@ -640,3 +640,14 @@ def test_eq13_mode(sk, oracle, T, F, E, M):
         sk14 = sk.sk_frame(d, M, **kw).SK.cpu().numpy().astype(np.float64)
         c = (M * N + 1.0) * (M - 1.0) / ((M * N - 1.0) * (M + 1.0))
         np.testing.assert_allclose(got, c * sk14, rtol=2e-6, atol=2e-7)
+
+
+def test_measurement_entries(sk):
+    """sk_debug_loop_ceiling / sk_debug_pipe_rate (measurement only): they run and return plausible
+    cycle counts (one instruction per 1..4 cycles; the loop's 3.98 instructions per 32 samples cannot
+    take fewer than 3.98 cycles)."""
+    c = sk.sk_debug_loop_ceiling(12, 20)
+    assert 3.98 < c < 12.0
+    for mode, name in enumerate(sk.PIPE_MODES):
+        r = sk.sk_debug_pipe_rate(mode, 16)
+        assert 0.9 < r < 8.0, (name, r)
