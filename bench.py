@@ -135,7 +135,21 @@ def run_ceiling(args):
     pts = [{"warps_per_sm": w, "subpartition_cycles_per_32_samples": sk.sk_debug_loop_ceiling(w, 200, dev)}
            for w in (4, 8, 12, 16)]
     pipes = {name: sk.sk_debug_pipe_rate(m, 16, dev) for m, name in enumerate(sk.PIPE_MODES)}
+    # the loop alone for ~1.5 s with the NVML record: what the arithmetic draws without any memory traffic
+    sampler = ClockSampler(0)
+    sampler.start()
+    t_lo = time.perf_counter()
+    sampler.window = (t_lo, None)
+    cyc_long, calls = [], 0
+    while time.perf_counter() - t_lo < 1.5:
+        cyc_long.append(sk.sk_debug_loop_ceiling(12, 4000, dev))
+        calls += 1
+    t_hi = time.perf_counter()
+    sampler.window = (t_lo, t_hi)
+    loop_clocks = sampler.summary()
+    sampler.stop_flag = True
     subp = 4 * torch.cuda.get_device_properties(dev).multi_processor_count
+    loop_rate = subp * 32 * (loop_clocks["sm_mhz"] or 1965) * 1e6 / (sum(cyc_long) / len(cyc_long))
     best = min(p["subpartition_cycles_per_32_samples"] for p in pts if p["warps_per_sm"] <= 12)
     print(json.dumps({
         "op": "ceiling", "metric": "sm_side_ceiling_samples_per_s", "value": subp * 32 * 1.965e9 / best, "unit": "samples/s",
@@ -144,7 +158,11 @@ def run_ceiling(args):
                    "value_is": "sub-partitions x 32 lanes x 1.965 GHz / cycles per 32 samples at 12 warps per SM",
                    "points": pts,
                    "subpartition_cycles_per_warp_instruction": pipes,
-                   "pipes_note": "16 warps per SM, 8 independent chains per lane; pairs count two instructions"},
+                   "pipes_note": "16 warps per SM, 8 independent chains per lane; pairs count two instructions",
+                   "loop_for_1.5_s": {"clocks": loop_clocks, "samples_per_s": loop_rate,
+                                      "pj_per_sample": (loop_clocks["power_w"] or 0) / loop_rate * 1e12,
+                                      "note": "12 warps per SM, back-to-back launches: board power of the arithmetic "
+                                              "alone (no HBM traffic), idle power included"}},
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
