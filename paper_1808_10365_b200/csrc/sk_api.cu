@@ -124,6 +124,20 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     const bool grid_ok = B / bpu <= 65535u && F <= 65535u && (unsigned long long)F * E < (1ull << 32) &&
                          (unsigned long long)B * M < (1ull << 31);
     pl.chunk = (pl.vec && grid_ok && pl.L >= 4) ? chunk_rows(M, pl.L) : 0u;
+    if (pl.chunk == 0u && pl.vec && grid_ok && g_force_lanes.load(std::memory_order_relaxed) == 0) {
+        // the block length is not a whole number of tiles at this slab width (a tile is 8 KiB: 32 rows of
+        // 256 B, 64 of 128 B, 128 of 64 B): a wider slab has shorter tiles; take the first width that fits
+        for (int L2 = 16; L2 >= 4; L2 >>= 1) {
+            if ((uint32_t)L2 > E / 16 || L2 == pl.L || chunk_rows(M, L2) == 0u) continue;
+            pl.L = L2;
+            pl.slabs = (cover + 16u * L2 - 1) / (16u * L2);
+            const uint32_t it2 = (M + 32u / L2 - 1) / (32u / L2);
+            pl.wide = it2 <= sk::AccWide2::kMaxSamples;
+            pl.chain = it2 <= sk::AccChain2::kMaxSamples;
+            pl.chunk = chunk_rows(M, L2);
+            break;
+        }
+    }
     return pl;
 }
 
