@@ -94,6 +94,7 @@ struct Plan {
     bool chain;           // AccChain2 usable by the direct-load kernel (samples per lane <= 128)
     uint32_t chunk;       // stream kernel: rows per read-out, 0 = stream kernel not usable
     uint32_t bpu;         // stream kernel: M-row blocks per unit (a power of two dividing B, >= 1 << (nlev-1))
+    uint32_t ragged_tpb;  // != 0: the ragged stream kernel runs, with this many tiles per block (chunk == 0)
 };
 
 // nlev = integration lengths wanted (M << 0 .. M << (nlev-1)); B % (1 << (nlev-1)) == 0.
@@ -138,6 +139,23 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
             break;
         }
     }
+    if (pl.chunk == 0u && pl.vec && grid_ok && nlev == 1) {
+        // no slab width makes the block a whole number of tiles: the ragged stream kernel, at the widest
+        // slab (shortest tiles), as long as the block is at least two tiles long
+        int L2 = g_force_lanes.load(std::memory_order_relaxed) ? pl.L : 16;
+        while (L2 > 1 && (uint32_t)L2 > E / 16) L2 >>= 1;
+        const uint32_t R = sk::kTileBytes / (16u * (uint32_t)L2);
+        const uint32_t it2 = (M + 32u / L2 - 1) / (32u / L2);            // samples a lane adds per block
+        // worth it for long blocks only: up to 128 samples per lane the direct-load kernel keeps the packed
+        // accumulators and is as fast (measured: M = 100, 250: 4.2-4.7 TB/s either way; M = 1000: 5.0 against 3.7)
+        if (L2 >= 4 && M >= 2u * R && it2 > sk::AccChain2::kMaxSamples) {
+            pl.L = L2;
+            pl.slabs = (cover + 16u * L2 - 1) / (16u * L2);
+            pl.wide = it2 <= sk::AccWide2::kMaxSamples;
+            pl.chain = false;
+            pl.ragged_tpb = (M + R - 1) / R;
+        }
+    }
     return pl;
 }
 
@@ -177,7 +195,7 @@ EncodeTiledFn encode_tiled() {
 // The stream kernel runs whenever it applies; sk_debug_set_plan(SK_PLAN_LDG, ..) turns it off.
 bool stream_wanted(const Plan& pl) {
     if (g_force_path.load(std::memory_order_relaxed) == SK_PLAN_LDG) return false;
-    return pl.chunk != 0 && encode_tiled() != nullptr;
+    return (pl.chunk != 0 || pl.ragged_tpb != 0) && encode_tiled() != nullptr;
 }
 
 template <int L, int NLEV, bool CHUNKED>
@@ -207,6 +225,31 @@ int launch_stream_K(const CUtensorMap& tmap, const sk::FrameParams& p, uint32_t 
 }
 
 template <int L>
+int launch_ragged_L(const CUtensorMap& tmap, const sk::FrameParams& p, uint32_t zblocks, cudaStream_t st) {
+    static std::atomic<bool> attr_set[kMaxDevices];
+    const int dev = current_device();
+    if (!attr_set[dev].load(std::memory_order_acquire)) {
+        cudaFuncSetAttribute(sk::sk_stream_ragged_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sk::kStreamSmemBytes);
+        cudaFuncSetAttribute(sk::sk_stream_ragged_kernel<L>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
+        attr_set[dev].store(true, std::memory_order_release);
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.slabs, p.F, zblocks);
+    cfg.blockDim = dim3(32);
+    cfg.dynamicSmemBytes = sk::kStreamSmemBytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, sk::sk_stream_ragged_kernel<L>, tmap, p);
+    return e == cudaSuccess ? SK_OK : (int)e;
+}
+
+template <int L>
 int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, bool chunked, uint32_t zblocks,
                     cudaStream_t st) {
     switch (p.nlev) {
@@ -232,6 +275,15 @@ int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     const bool chunked = pl.chunk != p.M;
     const uint32_t zblocks = p.B / pl.bpu;
     int rc;
+    if (pl.ragged_tpb) {
+        switch (pl.L) {
+            case 16: rc = launch_ragged_L<16>(tmap, p, zblocks, st); break;
+            case 8:  rc = launch_ragged_L<8>(tmap, p, zblocks, st); break;
+            default: rc = launch_ragged_L<4>(tmap, p, zblocks, st); break;
+        }
+        if (rc == SK_OK) ++g_launches;
+        return rc;
+    }
     switch (pl.L) {
         case 16: rc = launch_stream_L<16>(tmap, p, chunked, zblocks, st); break;
         case 8:  rc = launch_stream_L<8>(tmap, p, chunked, zblocks, st); break;
@@ -249,7 +301,8 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
         if (stream_wanted(pl)) {
             p.chunk = pl.chunk;
             p.bpu = pl.bpu;
-            p.unit_tiles = p.M * pl.bpu / (sk::kTileBytes / (16u * pl.L));
+            p.tpb = pl.ragged_tpb;
+            p.unit_tiles = pl.ragged_tpb ? pl.ragged_tpb * pl.bpu : p.M * pl.bpu / (sk::kTileBytes / (16u * pl.L));
             const int rc = launch_stream(pl, p, st);
             if (rc != SK_OK) return rc;
         } else if (pl.chain) launch_vec_L<sk::AccChain2>(pl.L, p, st);
@@ -608,7 +661,7 @@ int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t f
     const Plan pl = make_plan(nullptr, E, M, T / M, F, nullptr, first_n, false, (flags & SK_FRAME_INPUTS_READY) != 0, nlev);
     plan4[0] = (uint32_t)pl.L;
     plan4[1] = pl.slabs;
-    plan4[2] = (pl.vec && stream_wanted(pl)) ? pl.chunk : 0u;
+    plan4[2] = (pl.vec && stream_wanted(pl)) ? (pl.ragged_tpb ? sk::kRaggedTilesPerReadout * sk::kTileBytes / (16u * pl.L) : pl.chunk) : 0u;
     plan4[3] = pl.bpu;
     return SK_OK;
 }

@@ -44,6 +44,7 @@ struct FrameParams {
     uint32_t chunk;           // stream kernel: rows per accumulator read-out (divides M)
     uint32_t bpu;             // stream kernel: M-row blocks per unit (a multiple of 1 << (nlev-1))
     uint32_t unit_tiles;      // stream kernel: TMA tiles per unit = M * bpu / (rows per tile)
+    uint32_t tpb;             // ragged stream kernel: tiles per block = ceil(M / rows per tile); unit_tiles = tpb * bpu
     uint32_t slabs;           // units per cell that are launched
     uint32_t nunits;          // cells * slabs
 };

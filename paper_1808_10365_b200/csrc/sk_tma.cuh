@@ -215,4 +215,120 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same kernel for a block length that is NOT a whole number of tiles (M = 250, 1000, ...): a
+// block is tpb = ceil(M / R) tiles, the last of them partial.  Every block's first tile starts at the
+// block's first row (a TMA box may start at any row), the partial tile is fetched whole (its surplus
+// rows belong to the next block, or lie beyond T and come back as zeros) and only its first
+// M - (tpb-1) R rows are added; the accumulators are read out every 8 tiles (128 samples per lane)
+// and at every block end.  One integration length, chunked running sums; everything after the
+// row loop is the code of sk_stream_kernel.  The host uses it when M >= 2 R (at most a third of
+// the fetched rows are surplus); shorter ragged blocks take the direct-load kernel.
+constexpr int kRaggedTilesPerReadout = 8;
+
+template <int L>
+__global__ void __maxnreg__(128)
+sk_stream_ragged_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) {
+    constexpr int RPW = 32 / L;
+    constexpr int W = 16 * L;
+    constexpr int R = kTileBytes / W;
+    constexpr int NLD = R / RPW;
+    constexpr int kOwn = Owned<L>::value;
+    static_assert(kRaggedTilesPerReadout * NLD <= (int)AccChain2::kMaxSamples, "read-out interval");
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x;
+    const uint32_t ring = smem_addr(smem);
+    const uint32_t bars = ring + kStages * kTileBytes;
+    const uint32_t slab = blockIdx.x, f = blockIdx.y;
+    const uint32_t x0 = f * p.E + slab * W;
+    const uint32_t tpb = p.tpb, total = p.unit_tiles;          // tiles per block, tiles of this unit (tpb * bpu)
+    const uint32_t last_rows = p.M - (tpb - 1u) * R;            // rows of a block's last tile that belong to it
+
+    asm volatile("griddepcontrol.launch_dependents;");
+    if (!p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");
+
+    // producer (lane 0): the next tile to request is tile pk of the block that starts at row py
+    uint32_t pk = 0, py = blockIdx.z * p.M * p.bpu;
+    auto request = [&](uint32_t stage) {
+        mbar_expect_tx(bars + 8 * stage, kTileBytes);
+        tma_load_tile(ring + stage * kTileBytes, &tmap, x0, py + pk * R, bars + 8 * stage);
+        if (++pk == tpb) { pk = 0; py += p.M; }
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+#pragma unroll
+        for (int s = 0; s < kStages; ++s)
+            if ((uint32_t)s < total) request(s);
+    }
+    __syncwarp();
+
+    const int cl = lane % L, r0 = lane / L;
+    const uint32_t lane_off = r0 * W + cl * 16;
+    const uint32_t e0 = (slab * L + cl) * 16u;
+    const bool active = e0 < p.E;
+    const bool owner = (RPW <= 16) || (r0 < 16);
+
+    UnpackConsts kc;
+    kc.init();
+    AccChain2 acc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k].reset();
+    uint32_t run1[kOwn], run2[kOwn];
+#pragma unroll
+    for (int i = 0; i < kOwn; ++i) run1[i] = run2[i] = 0;
+
+    uint32_t s = 0, parity = 0, tc = 0, k = 0, blk = 0;
+    for (uint32_t g = 0; g < total; ++g) {
+        const uint32_t src = ring + s * kTileBytes + lane_off;
+        mbar_wait(bars + 8 * s, parity);
+        if (k + 1u < tpb || last_rows == (uint32_t)R) {
+#pragma unroll
+            for (int i = 0; i < NLD; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+        } else {
+            // the block's last tile: row i * RPW + r0 of the tile counts only while it is below last_rows
+            for (uint32_t i = 0; i * RPW + (uint32_t)r0 < last_rows; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+        }
+        __syncwarp();
+        if (lane == 0 && g + kStages < total) request(s);
+        if (++s == kStages) { s = 0; parity ^= 1; }
+        const bool block_end = ++k == tpb;
+        if (++tc < (uint32_t)kRaggedTilesPerReadout && !block_end) continue;
+        tc = 0;
+
+        uint32_t S1[16], S2[16];
+        read16(acc, 0u, S1, S2);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[i].reset();
+        if (!active) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { S1[i] = 0; S2[i] = 0; }
+        }
+        const int base = reduce_scatter_rows<L>(S1, S2, r0);
+        const uint32_t e_first = e0 + base;
+#pragma unroll
+        for (int i = 0; i < kOwn; ++i) { run1[i] += S1[i]; run2[i] += S2[i]; }
+        if (!block_end) continue;
+        k = 0;
+
+        // ---- a block of M rows is complete
+        if (p.inputs_ready) asm volatile("griddepcontrol.wait;" ::: "memory");   // before the first write
+        const uint32_t b0 = blockIdx.z * p.bpu + blk;
+        if (p.S1out && active && owner) {
+            const size_t cell = (size_t)b0 * p.F + f;
+            uint32_t* o1 = p.S1out + cell * p.E + e_first;
+            uint32_t* o2 = p.S2out + cell * p.E + e_first;
+#pragma unroll
+            for (int i = 0; i < kOwn; ++i) { o1[i] = run1[i]; o2[i] = run2[i]; }
+        }
+        if (p.lev[0].SK)
+            publish_and_finalize(p, 0, b0, f, slab, lane, unit_partial<L>(p, (double)p.M, active, owner, e_first, run1, run2));
+#pragma unroll
+        for (int i = 0; i < kOwn; ++i) run1[i] = run2[i] = 0;
+        ++blk;
+    }
+}
+
 }  // namespace sk

@@ -68,6 +68,8 @@ SHAPES = [
     (4096, 2, 2048, 32), (2048, 1, 4096, 64),
     # block lengths that are whole tiles only at the widest slab (32 rows x 256 B): the plan widens the slab
     (768, 1, 2048, 96), (1120, 2, 512, 160),
+    # long blocks that are not a whole number of tiles at any width: the ragged stream kernel (partial last tile)
+    (3000, 2, 2048, 300), (2000, 1, 528, 1000), (4 * 1025, 1, 2048, 1025),
     # beyond the stream kernel: more than 65535 units along time (grid.z), tiny E, and a block
     # length with no usable divisor (direct-load kernel)
     (140000, 1, 16, 2), (16384, 1, 32, 8192), (65536, 1, 48, 32768), (2 * 4099, 1, 256, 4099),
