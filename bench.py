@@ -272,11 +272,13 @@ def run_reference(args):
     host = sk_synth.make_frame(sub).numpy()
     steps = max(1, min(args.steps, 20))
     warm = max(0, min(args.warmup, 5))
+    n_sigma = 5.0                                          # as the GPU arm
+    sk_mean = round(float(sk_oracle.frame(null_frame(sk_synth, cfg, cfg.M).numpy(), cfg.M)["SK"].astype("float64").mean()), 4)
     for _ in range(warm):
-        sk_oracle.frame(host, cfg.M, n_sigma=cfg.n_sigma)
+        sk_oracle.frame(host, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean)
     t0 = time.perf_counter()
     for _ in range(steps):
-        sk_oracle.frame(host, cfg.M, n_sigma=cfg.n_sigma)
+        sk_oracle.frame(host, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean)
     dt = time.perf_counter() - t0
     v = host.size * steps / dt
     line = {
@@ -284,7 +286,7 @@ def run_reference(args):
         "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "N": cfg.E,
-                   "n_sigma": cfg.n_sigma, "zero_flagged": False,
+                   "n_sigma": n_sigma, "sk_mean": sk_mean, "zero_flagged": False,
                    "sample": f"{blocks} of {cfg.B} blocks per step ({host.size} samples)"},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                          "sample": f"{steps} steps x {host.size} samples of {cfg.name}"},
@@ -401,9 +403,15 @@ def null_mean(sk, sk_synth, cfg, dev, M=None):
     """The flag centre the paper's way: mean SK of an RFI-free simulation with the
     workload's per-input sigmas (the 4-bit null mean is not 1: App. B)."""
     M = M or cfg.M
-    null = sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * M), M=M, cw_block_inputs=None, cw_freqs=(),
-                                         burst_fraction=0.0, sine_freqs=()), device=dev, frame=777)
-    return float(sk.sk_frame(null, M).SK.double().mean().item())
+    null = null_frame(sk_synth, cfg, M).to(dev)
+    return round(float(sk.sk_frame(null, M).SK.double().mean().item()), 4)
+
+
+def null_frame(sk_synth, cfg, M):
+    """The RFI-free simulation both arms centre their flag on: drawn on the CPU, so that the GPU arm and the
+    reference arm see the same bytes (and print the same sk_mean, rounded to 1e-4)."""
+    return sk_synth.make_frame(cfg.with_(T=min(cfg.T, 8 * M), M=M, cw_block_inputs=None, cw_freqs=(),
+                                         burst_fraction=0.0, sine_freqs=()), frame=777)
 
 
 def timed_replays(torch, graph, stream, seconds, step_s_estimate, steps_per_replay, barrier, sampler=None):
