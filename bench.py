@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling"],
+    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling", "fig5", "fig6"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
@@ -357,6 +357,68 @@ def run_cm(args):
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
+def run_fig5(args):
+    """--op fig5: App. A / Fig. 5 of the paper on the device: variance of SK~ over 1000
+    datasets of n = 256 samples x N receivers against the amplitude of a common-mode signal, and the
+    effective number of receivers N_eff = 4 / (n var)."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    torch.cuda.set_device(0)
+    D, n = 1000, 256
+    amps = (0.0, 0.03, 0.1, 0.3, 1.0, 3.0)
+    n0 = sk.sk_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    rows = []
+    for N in (128, 256, 512, 1024, 2048, 4096):
+        pts = []
+        for a in amps:
+            mean, var = sk.sk_moments(sk.sk_sim_common_mode(D, n, N, a, seed=1808 + N))
+            v = float(var[0].item())
+            pts.append({"amp": a, "mean": float(mean[0].item()), "var": v, "n_eff": 4.0 / (n * v)})
+        rows.append({"N": N, "var_predicted_independent": 4.0 / (n * N), "points": pts})
+    e1.record()
+    torch.cuda.synchronize()
+    total = sum(D * n * r["N"] * len(amps) for r in rows)
+    print(json.dumps({
+        "op": "fig5", "metric": "simulated_samples_per_s", "value": total / (e0.elapsed_time(e1) * 1e-3), "unit": "samples/s",
+        "n_gpus": 1, "steps": 1, "warmup": 0, "ms_per_step": e0.elapsed_time(e1), "higher_is_better": True,
+        "data": "synthetic", "dtype": "f64",
+        "config": {"workload": f"App. A / Fig. 5: {D} datasets x n={n}, x = z + amp*c, variance of SK~ and N_eff = 4/(n var)",
+                   "var_predicted_single_receiver": 4.0 / n, "table": rows},
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
+def run_fig6(args):
+    """--op fig6: App. B / Fig. 6 on the device: moments of SK~ on 4+4-bit data with an
+    RMS of 1.52 LSB per component against the same moments of float ('non-digitised') Gaussian data, for
+    M = 256 and N = 16 ... 2048 combined receivers."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    torch.cuda.set_device(0)
+    M, E, B = 256, 2048, 1024
+    thr = sk_synth.digitiser_thresholds(torch.full((E,), 1.52, dtype=torch.float64)).cuda()
+    n0 = sk.sk_launch_count()
+    data = sk.sk_sim_digitised(B * M, 1, E, thr, seed=6, frame=0)
+    rows = []
+    for N in (16, 64, 256, 1024, 2048):
+        mean, var = sk.sk_moments(sk.sk_frame(data, M, first_n=N).SK)
+        fm, fv = sk.sk_moments(sk.sk_sim_common_mode(B, M, N, 0.0, seed=66 + N))
+        rows.append({"N": N, "digitised_mean": float(mean[0].item()), "float_mean": float(fm[0].item()),
+                     "mean_difference": float(mean[0].item()) - float(fm[0].item()),
+                     "digitised_var_over_4_MN": float(var[0].item()) * M * N / 4.0,
+                     "float_var_over_4_MN": float(fv[0].item()) * M * N / 4.0})
+    torch.cuda.synchronize()
+    print(json.dumps({
+        "op": "fig6", "metric": "null_mean_offset", "value": rows[-1]["mean_difference"], "unit": "SK", "n_gpus": 1,
+        "steps": 1, "warmup": 0, "higher_is_better": False, "data": "synthetic", "dtype": "u8 / f64",
+        "config": {"workload": f"App. B / Fig. 6: {B} blocks of M={M} x E={E}, 4+4-bit round-and-clip Gaussian, RMS 1.52 LSB "
+                               "(sk_sim_digitised -> sk_frame -> sk_moments) against float Gaussian data (sk_sim_common_mode, amp 0)",
+                   "value_is": "digitised - float mean of SK~ at N = 2048", "table": rows},
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
 def run_aux(args):
     """--op rebin|single: one of the small HBM-bound kernels beside the hot path, on S1/S2 arrays of
     config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), two rotating copies."""
@@ -569,6 +631,10 @@ def main():
         return run_multi(args)
     if args.op == "ceiling":
         return run_ceiling(args)
+    if args.op == "fig5":
+        return run_fig5(args)
+    if args.op == "fig6":
+        return run_fig6(args)
     if args.op != "frame":
         return run_aux(args)
 
