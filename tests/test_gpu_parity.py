@@ -655,3 +655,20 @@ def test_measurement_entries(sk):
     for mode, name in enumerate(sk.PIPE_MODES):
         r = sk.sk_debug_pipe_rate(mode, 16)
         assert 0.9 < r < 8.0, (name, r)
+
+
+@pytest.mark.parametrize("first_n", [16, 64, 300, 2048])
+def test_first_n_without_sums_and_excision(sk, oracle, vector_path, first_n):
+    """The launch the sweep times: no sums requested, so only the slabs that cover first_n are
+    read — but a flagged cell is excised over ALL E inputs (A11), and SK / mask are the oracle's."""
+    T, F, E, M = 2048, 2, 2048, 256
+    data = sk_synth.random_bytes(T, F, E, seed=77)
+    data[M:2 * M, 1, :] = 0x88                                  # an all-zero cell: SK = 0, flagged
+    ref = oracle.frame(data.numpy(), M, first_n=first_n, n_sigma=3.0, sk_mean=0.45, zero_flagged=True)
+    d = data.cuda()
+    out = sk.sk_frame(d, M, first_n=first_n, n_sigma=3.0, sk_mean=0.45, zero_flagged=True)
+    torch.cuda.synchronize()
+    assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
+    np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])
+    assert ref["mask"].sum() > 0
