@@ -672,3 +672,23 @@ def test_first_n_without_sums_and_excision(sk, oracle, vector_path, first_n):
     np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
     np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])
     assert ref["mask"].sum() > 0
+
+
+def test_ragged_blocks_pipelined_with_excision(sk, oracle):
+    """Long blocks that are not a whole number of tiles (the ragged stream kernel), back to back with
+    SK_FRAME_INPUTS_READY and in-place excision: every frame's SK, mask and bytes are the oracle's."""
+    T, F, E, M = 3000, 2, 2048, 300
+    assert sk.sk_debug_get_plan(T, F, E, M, inputs_ready=True)[2] != 0          # a TMA kernel, not the direct-load one
+    frames = [sk_synth.random_bytes(T, F, E, seed=300 + i) for i in range(4)]
+    for fr in frames:
+        fr[M:2 * M, 0, :] = 0x88
+    work = [fr.cuda() for fr in frames]
+    ws = sk.workspace_for(T, F, E, M, work[0].device, 3003)
+    outs = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, zero_flagged=True, inputs_ready=True, workspace=ws) for d in work]
+    torch.cuda.synchronize()
+    assert int(ws.abs().sum().item()) == 0
+    for fr, d, o in zip(frames, work, outs):
+        ref = oracle.frame(fr.numpy(), M, n_sigma=2.0, sk_mean=0.4, zero_flagged=True)
+        assert_sk_close(o.SK.cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(o.mask.cpu().numpy(), ref["mask"])
+        np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])
