@@ -128,7 +128,9 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     if (pl.chunk == 0u && pl.vec && grid_ok && g_force_lanes.load(std::memory_order_relaxed) == 0) {
         // the block length is not a whole number of tiles at this slab width (a tile is 8 KiB: 32 rows of
         // 256 B, 64 of 128 B, 128 of 64 B): a wider slab has shorter tiles; take the first width that fits
-        for (int L2 = 16; L2 >= 4; L2 >>= 1) {
+        int widest = 16;                                  // ... but no wider than the receivers asked for justify
+        while (widest > 4 && 8u * widest >= cover) widest >>= 1;
+        for (int L2 = widest; L2 >= 4; L2 >>= 1) {
             if ((uint32_t)L2 > E / 16 || L2 == pl.L || chunk_rows(M, L2) == 0u) continue;
             pl.L = L2;
             pl.slabs = (cover + 16u * L2 - 1) / (16u * L2);
@@ -144,6 +146,7 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
         // slab (shortest tiles), as long as the block is at least two tiles long
         int L2 = g_force_lanes.load(std::memory_order_relaxed) ? pl.L : 16;
         while (L2 > 1 && (uint32_t)L2 > E / 16) L2 >>= 1;
+        while (L2 > 4 && 8u * L2 >= cover && g_force_lanes.load(std::memory_order_relaxed) == 0) L2 >>= 1;
         const uint32_t R = sk::kTileBytes / (16u * (uint32_t)L2);
         const uint32_t it2 = (M + 32u / L2 - 1) / (32u / L2);            // samples a lane adds per block
         // worth it for long blocks only: up to 128 samples per lane the direct-load kernel keeps the packed
