@@ -35,8 +35,13 @@ def lib() -> C.CDLL:
     if _lib is not None:
         return _lib
     if not os.path.exists(LIB_PATH):
-        raise SKError(f"{LIB_PATH} is missing: build it with `python -m paper_1808_10365_b200.build` "
-                      "(there is no CPU fallback)")
+        # a fresh checkout: compile the library in-tree (nvcc), then load it; there is no other path
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as e:
+            raise SKError(f"{LIB_PATH} is missing and could not be built ({e}): run "
+                          "`python -m paper_1808_10365_b200.build` (there is no CPU fallback)") from e
     L = C.CDLL(LIB_PATH)
     u32, vp, f32, i32, sz = C.c_uint32, C.c_void_p, C.c_float, C.c_int, C.c_size_t
     L.sk_power_sums.argtypes = [vp, u32, u32, u32, u32, vp, vp, vp]
