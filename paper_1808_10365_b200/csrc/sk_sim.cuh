@@ -27,28 +27,23 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// value + 8 = 1 + #{ j : u >= thr[j] }  (value = -7 + count).  The thresholds ascend, so the count
-// is found by a 4-step binary search (the caller's table is a CDF): 4 compares and 11 selects on
-// registers instead of 14 compare-adds.  (Equal neighbouring thresholds are fine: the count is the
-// number of thresholds <= u either way.)
-__device__ __forceinline__ uint32_t digitise_nibble(uint32_t u, const uint32_t (&thr)[14]) {
-    // n = number of thresholds known to be <= u; thr[14], thr[15] are +infinity (never selected as true)
-    uint32_t n = (u >= thr[7]) ? 8u : 0u;
-    const uint32_t t4 = n ? thr[11] : thr[3];
-    n += (u >= t4) ? 4u : 0u;
-    // n in {0, 4, 8, 12}: next probe thr[n + 1]; at n = 12 that is thr[13]
-    const uint32_t a2 = (n & 4u) ? ((n & 8u) ? thr[13] : thr[5]) : ((n & 8u) ? thr[9] : thr[1]);
-    const uint32_t n2 = n + ((u >= a2) ? 2u : 0u);
-    // at n = 12 the probe was thr[13] itself: the count is 13 or 14, decided by thr[12] and thr[13]
-    if (n == 12u) return 1u + 12u + ((u >= thr[12]) ? 1u : 0u) + ((u >= thr[13]) ? 1u : 0u);
-    // n2 in {0, 2, ..., 10}: last probe thr[n2]
-    uint32_t t1 = thr[0];
-#pragma unroll
-    for (int k = 2; k <= 10; k += 2) t1 = (n2 == (uint32_t)k) ? thr[k] : t1;
-    return 1u + n2 + ((u >= t1) ? 1u : 0u);
+// value + 8 = 1 + #{ j : u >= thr[j] }  (value = -7 + count).  The thresholds ascend (the caller's table is a
+// CDF), so the count is found by a 4-step branch-free binary search.  The table lives in shared memory as
+// col[k * kSimStride] (k = 0..14, entry 14 = 0xFFFFFFFF), one column per thread and receiver, so that a warp's
+// reads never conflict whatever the indices are; the ALU pipe (ISETP / SEL at half rate) is what bounds this
+// kernel, and the search costs it 3 instructions per step instead of the 23 per component of a search over
+// registers (select chains).  Equal neighbouring thresholds are fine: the count is the number of thresholds <= u.
+constexpr int kSimThreads = 128;
+constexpr int kSimStride = 2 * kSimThreads;     // words between consecutive thresholds of one column
+
+__device__ __forceinline__ uint32_t digitise_nibble(uint32_t u, const uint32_t* col) {
+    uint32_t n = (u >= col[7 * kSimStride]) ? 8u : 0u;
+    n += (u >= col[(n + 3u) * kSimStride]) ? 4u : 0u;
+    n += (u >= col[(n + 1u) * kSimStride]) ? 2u : 0u;
+    n += (u >= col[n * kSimStride]) ? 1u : 0u;           // n = 14 reads the pad: u = 2^32 - 1 would count it
+    return 1u + (n < 14u ? n : 14u);
 }
 
-constexpr int kSimThreads = 128;
 constexpr int kSimRows = 64;              // rows per thread (at least)
 
 // Thread = one receiver pair (2j, 2j+1) for rpt rows r = t*F + f; counter (j, r, frame), key seed.
@@ -59,11 +54,13 @@ sk_sim_kernel(uint8_t* __restrict__ data, uint64_t rows, uint32_t rpt, uint32_t 
     const uint32_t e = 2 * j;
     if (e >= E) return;
     const bool two = e + 1 < E;
-    uint32_t ta[14], tb[14];
+    __shared__ uint32_t table[15 * kSimStride];
+    uint32_t* const ta = table + threadIdx.x;                      // receiver 2j
+    uint32_t* const tb = table + kSimThreads + threadIdx.x;        // receiver 2j + 1
 #pragma unroll
-    for (int i = 0; i < 14; ++i) {
-        ta[i] = __ldg(thr + (size_t)e * 14 + i);
-        tb[i] = two ? __ldg(thr + (size_t)(e + 1) * 14 + i) : 0u;
+    for (int i = 0; i < 15; ++i) {
+        ta[i * kSimStride] = i < 14 ? __ldg(thr + (size_t)e * 14 + i) : 0xFFFFFFFFu;
+        tb[i * kSimStride] = (i < 14 && two) ? __ldg(thr + (size_t)(e + 1) * 14 + i) : 0xFFFFFFFFu;
     }
     const uint64_t r0 = (uint64_t)blockIdx.y * rpt;
     const uint64_t r1 = r0 + rpt < rows ? r0 + rpt : rows;
