@@ -692,3 +692,42 @@ def test_ragged_blocks_pipelined_with_excision(sk, oracle):
         assert_sk_close(o.SK.cpu().numpy(), ref["SK"])
         np.testing.assert_array_equal(o.mask.cpu().numpy(), ref["mask"])
         np.testing.assert_array_equal(d.cpu().numpy(), ref["data"])
+
+
+def test_randomised_shapes_and_flags(sk, oracle):
+    """Seeded random walk over the call's whole argument space — block lengths of every kind (whole
+    tiles, ragged, tiny, long), E with and without the vector path, receiver selection, excision, sums,
+    SK_FRAME_INPUTS_READY, both vector kernels and forced slab widths — each case against the oracle."""
+    rng = np.random.default_rng(12345)
+    for it in range(80):
+        M = int(rng.choice([2, 7, 16, 32, 33, 64, 96, 100, 128, 160, 250, 256, 300, 512, 1000, 1024, 1025, 2048, 4099]))
+        B, F = int(rng.integers(1, 9)), int(rng.integers(1, 4))
+        E = int(rng.choice([16, 32, 48, 64, 96, 128, 256, 272, 512, 528, 1024, 2048, 2064, 4096, 37, 100]))
+        if B * M * F * E > 32 << 20:
+            B = max(1, (32 << 20) // (M * F * E))
+        T = B * M
+        data = sk_synth.random_bytes(T, F, E, seed=int(rng.integers(1 << 30)))
+        if rng.random() < 0.3:
+            data[:M, 0, : max(1, E // 3)] = 0x88
+        kw, r = {}, rng.random()
+        if r < 0.3:
+            kw["first_n"] = int(rng.integers(1, E + 1))
+        elif r < 0.5:
+            sub = rng.random(E) < rng.random()
+            sub[int(rng.integers(E))] = True
+            kw["subset"] = sub
+        zero, sums, ready = bool(rng.random() < 0.5), bool(rng.random() < 0.5), bool(rng.random() < 0.5)
+        path, lanes = int(rng.choice([0, 0, 0, 1])), int(rng.choice([0, 0, 0, 16, 8, 4, 2, 1]))
+        sk_mean, ns = float(rng.choice([0.4, 0.9, 1.0])), float(rng.choice([1.0, 3.0]))
+        sk.sk_debug_set_plan(path, lanes)
+        ref = oracle.frame(data.numpy(), M, n_sigma=ns, sk_mean=sk_mean, zero_flagged=zero, **kw)
+        d = data.cuda()
+        out = sk.sk_frame(d, M, n_sigma=ns, sk_mean=sk_mean, zero_flagged=zero, want_sums=sums, inputs_ready=ready, **kw)
+        torch.cuda.synchronize()
+        case = (it, T, F, E, M, sorted(kw), zero, sums, ready, path, lanes)
+        np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"], err_msg=str(case))
+        np.testing.assert_array_equal(d.cpu().numpy(), ref["data"], err_msg=str(case))
+        assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
+        if sums:
+            np.testing.assert_array_equal(u32np(out.S1), ref["S1"], err_msg=str(case))
+            np.testing.assert_array_equal(u32np(out.S2), ref["S2"], err_msg=str(case))
