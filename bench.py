@@ -795,15 +795,18 @@ def main():
         "clocks": clocks,
     }
     if world == 1:
-        line["roofline"]["sm_ceiling"] = sm_ceiling(sk, torch, dev, (clocks or {}).get("sm_mhz"),
-                                                    (clocks or {}).get("sm_max_mhz"), value)
+        try:                                             # an extra: never let it cost the line
+            line["roofline"]["sm_ceiling"] = sm_ceiling(sk, torch, dev, (clocks or {}).get("sm_mhz"),
+                                                        (clocks or {}).get("sm_max_mhz"), value)
+        except Exception as e:
+            line["roofline"]["sm_ceiling"] = {"unavailable": str(e)}
     if args.zero:
         line["config"]["zero_note"] = ("the warm-up excises every frame once; the timed passes flag the same cells "
                                        "(their SK is 0) and overwrite them again: the traffic of a first pass")
     if burst is not None:
         burst["roofline_frac"] = burst["value"] * alg_bytes / frame_bytes / 1e9 / peak
         ceil = line["roofline"].get("sm_ceiling")
-        if ceil and (burst["clocks"] or {}).get("sm_mhz"):
+        if ceil and "subpartition_cycles_per_32_samples" in ceil and (burst["clocks"] or {}).get("sm_mhz"):
             burst["frac_of_sm_ceiling"] = burst["value"] * ceil["subpartition_cycles_per_32_samples"] / (
                 ceil["subpartitions"] * 32 * burst["clocks"]["sm_mhz"] * 1e6)
         line["burst"] = burst
