@@ -56,6 +56,7 @@ extern "C" {
 #define SK_ERR_N             -4   /* first_n == 0 or first_n > E (subset == NULL), or N == 0 */
 #define SK_ERR_PARAM         -5   /* n_sigma or sk_mean not finite, n_sigma < 0 */
 #define SK_ERR_WORKSPACE     -6   /* workspace NULL, misaligned (8 bytes) or too small */
+#define SK_ERR_SCRATCH       -7   /* sk_frame_noalloc: the shape needs more than SK_NOALLOC_SCRATCH_BYTES */
 
 /* a1-a3 (Eq. 7).  Reads data[T][F][E]; writes S1, S2 [T/M][F][E] (exact integers). */
 int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
@@ -100,6 +101,45 @@ int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
              const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
              int flags, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
              void* workspace, size_t workspace_bytes, void* stream);
+
+/* sk_frame for callers that cannot allocate device memory.
+ *
+ * Who that is: a stage plugged into a real-time correlator pipeline is usually handed its frame and
+ * output buffers by the host framework, which reserved the whole GPU at start-up and gives a stage no
+ * allocator of its own; a plug-in running inside somebody else's process may be forbidden to touch
+ * the device heap at all; and a frame loop that has gone real-time cannot afford cudaMalloc anyway,
+ * because it synchronises the device and stalls every other stage sharing the GPU.  sk_frame asks
+ * such a caller for a zero-filled workspace it has no way to provide.  This call does not: its
+ * workspace is an array of SK_NOALLOC_SCRATCH_BYTES built into the library's device image.  The
+ * caller passes only the frame and the outputs, exactly as for sk_frame; results are identical.
+ *
+ * What it costs and where the limit is: every GPU on which this library's kernels are loaded holds
+ * those SK_NOALLOC_SCRATCH_BYTES (4 MiB) from then until the process exits, whether or not this
+ * call is ever made.  A shape whose sk_frame_workspace_bytes(T, F, E, M) is larger (it grows as
+ * (T/M) * F * ceil(E/16) * 8 bytes: configs 0-2 of BASELINE.json fit, the 8 GiB frames of config 4
+ * do not) is refused with SK_ERR_SCRATCH before anything is enqueued; use sk_frame with a
+ * workspace from the framework's pool for those.
+ *
+ * The call itself never calls cudaMalloc, cudaFree or any library routine that allocates.  The
+ * first call made with a given device current also looks up the array's address on that device
+ * (cudaGetSymbolAddress, which may make the runtime load the library's kernels onto the device):
+ * make that first call during start-up, with the right device current, and before any stream
+ * capture begins; later calls on that device only enqueue work.
+ *
+ * Sharing: there is ONE array per device, used by every sk_frame_noalloc call of the process on
+ * that device, and it keeps what the last call left in it.  Each call therefore first clears the
+ * part it needs (a memset enqueued on `stream` ahead of the kernel), so a previous call of any
+ * shape, even a failed one, cannot disturb the result.  But two calls whose work overlaps on the
+ * GPU (different streams, or different host threads on different streams) race on the array and
+ * give wrong results: keep all sk_frame_noalloc calls of one device on one stream, or order
+ * them with events.  sk_frame with caller workspaces has no such restriction.
+ * Because of the clear, SK_FRAME_INPUTS_READY is accepted but buys no overlap with the previous
+ * kernel.  Arguments, flags, outputs and return values otherwise as for sk_frame. */
+#define SK_NOALLOC_SCRATCH_BYTES (4u << 20)
+int sk_frame_noalloc(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                     const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean,
+                     int flags, float* SK, uint8_t* mask, uint32_t* S1_opt, uint32_t* S2_opt,
+                     void* stream);
 
 /* Several integration lengths from ONE pass over HBM ("compute real-time SK
  * estimates at a variety of integration lengths"): the fused path at M, 2M, ..., M << (nlev-1),

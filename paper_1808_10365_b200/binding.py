@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
+           "sk_frame_noalloc",
            "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
            "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
            "sk_launch_count", "sk_debug_set_plan", "sk_debug_get_plan", "sk_debug_loop_ceiling", "sk_debug_pipe_rate")
@@ -50,6 +51,8 @@ def lib() -> C.CDLL:
     L.sk_frame_workspace_bytes.argtypes = [u32, u32, u32, u32]
     L.sk_frame_workspace_bytes.restype = sz
     L.sk_frame.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_frame_noalloc.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp]
+    L.sk_frame_noalloc.restype = i32
     L.sk_frame_host.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
     L.sk_frame_multi_workspace_bytes.argtypes = [u32, u32, u32, u32, u32]
     L.sk_frame_multi_workspace_bytes.restype = sz
@@ -366,6 +369,49 @@ def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: flo
                               flags, out.SK.data_ptr(), out.mask.data_ptr(), _ptr(out.S1), _ptr(out.S2),
                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
                               ts.cuda_stream), "sk_frame")
+    return out
+
+
+SK_NOALLOC_SCRATCH_BYTES = 4 << 20     # include/sk_b200.h
+
+
+def sk_frame_noalloc(data: torch.Tensor, M: int, out: SKResult, subset: Optional[torch.Tensor] = None, first_n=None,
+                     n_sigma: float = 3.0, sk_mean: float = 1.0, zero_flagged: bool = False, stream=None,
+                     eq13: bool = False) -> SKResult:
+    """sk_frame for code that must not allocate on the device (include/sk_b200.h, sk_frame_noalloc):
+    a pipeline stage whose buffers all come from the host framework's start-up pool, or a real-time
+    loop that cannot take the device-wide stall of a cudaMalloc.  The scratch is a 4 MiB array inside
+    the library, so frames whose sk_frame_workspace_bytes exceeds SK_NOALLOC_SCRATCH_BYTES raise.
+
+    Nothing is allocated here either, which is why `out` (SK, mask and optionally S1, S2, all
+    pre-allocated CUDA tensors of the right shape) is required and `subset`, if given, must already
+    be a uint8 [E] CUDA tensor.  All calls on one device share the one scratch array: keep them on
+    one stream.  Make the first call on a device before any stream capture (it looks up the array's
+    device address)."""
+    _dev(data, torch.uint8, "data")
+    T, F, E = data.shape
+    B = T // M if M else 0
+    _dev(out.SK, torch.float32, "out.SK")
+    _dev(out.mask, torch.uint8, "out.mask")
+    if tuple(out.SK.shape) != (B, F) or tuple(out.mask.shape) != (B, F):
+        raise SKError("out.SK and out.mask must be [T/M][F]")
+    for t, what in ((out.S1, "out.S1"), (out.S2, "out.S2")):
+        if t is not None:
+            _dev(t, torch.uint32, what)
+            if tuple(t.shape) != (B, F, E):
+                raise SKError(f"{what} must be [T/M][F][E]")
+    if subset is not None:
+        _dev(subset, torch.uint8, "subset")
+        if tuple(subset.shape) != (E,):
+            raise SKError("subset must have E entries")
+    elif first_n is None:
+        first_n = E
+    ts = _torch_stream(stream, data.device)
+    flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_EQ13 if eq13 else 0)
+    with torch.cuda.device(data.device):        # the scratch's address is looked up on the current device
+        _check(lib().sk_frame_noalloc(data.data_ptr(), T, F, E, M, _ptr(subset), int(first_n or 0), n_sigma, sk_mean,
+                                      flags, out.SK.data_ptr(), out.mask.data_ptr(), _ptr(out.S1), _ptr(out.S2),
+                                      ts.cuda_stream), "sk_frame_noalloc")
     return out
 
 

@@ -418,6 +418,38 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
 
 }  // namespace
 
+// ---- sk_frame_noalloc: the fused path for callers that cannot allocate ---------------------------
+// The scratch sk_frame otherwise takes from the caller (per-slab partial sums and per-cell arrival
+// counters) lives in this array instead.  It is part of the library's device image: every GPU on
+// which the library's kernels are loaded holds these SK_NOALLOC_SCRATCH_BYTES until the process exits.
+// In host code the name below is only a handle for the runtime, NOT a device address; the address is
+// asked for once per device (noalloc_scratch) and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char sk_noalloc_scratch[SK_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+// Device address of sk_noalloc_scratch on the CURRENT device, looked up on the first call made with
+// that device current and remembered afterwards (threads racing on the first call look up the same
+// address twice, nothing worse).  Returns a cudaError_t (> 0) if the runtime cannot resolve the symbol.
+int noalloc_scratch(void** out) {
+    static std::atomic<void*> cache[kMaxDevices];
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    const bool cached = dev >= 0 && dev < kMaxDevices;
+    void* ptr = cached ? cache[dev].load(std::memory_order_acquire) : nullptr;
+    if (!ptr) {
+        e = cudaGetSymbolAddress(&ptr, sk_noalloc_scratch);
+        if (e != cudaSuccess) return (int)e;
+        if (!ptr) return (int)cudaErrorInvalidSymbol;
+        if (cached) cache[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return SK_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int sk_power_sums(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
@@ -503,6 +535,29 @@ int sk_frame(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, cons
     if (!data || !SK || !mask) return SK_ERR_NULL;
     return frame_impl(data, T, F, E, M, 1, subset, first_n, n_sigma, &sk_mean, flags, &SK, &mask, S1_opt,
                       S2_opt, workspace, workspace_bytes_given, (cudaStream_t)stream);
+}
+
+int sk_frame_noalloc(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, const uint8_t* subset,
+                     uint32_t first_n, float n_sigma, float sk_mean, int flags, float* SK, uint8_t* mask,
+                     uint32_t* S1_opt, uint32_t* S2_opt, void* stream) {
+    if (!data || !SK || !mask) return SK_ERR_NULL;
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    // the size test comes before anything touches the device: a frame that does not fit is an
+    // argument error like any other
+    const size_t need = workspace_bytes(T / M, F, E, 1);
+    if (need > (size_t)SK_NOALLOC_SCRATCH_BYTES) return SK_ERR_SCRATCH;
+    // every other argument error too, so that "< 0 means nothing was enqueued" holds for the clear below
+    if (int rc = check_frame_args(subset, E, first_n, n_sigma, &sk_mean, 1, true)) return rc;
+    if ((S1_opt == nullptr) != (S2_opt == nullptr)) return SK_ERR_NULL;
+    void* scratch = nullptr;
+    if (int rc = noalloc_scratch(&scratch)) return rc;
+    // The array keeps whatever the last call left in it.  A completed call leaves zeros, one that
+    // failed half-way may not have, and the kernels count arrivals up from zero: clear the part this
+    // shape uses, in stream order, before the kernel.
+    const cudaError_t e = cudaMemsetAsync(scratch, 0, need, (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    return frame_impl(data, T, F, E, M, 1, subset, first_n, n_sigma, &sk_mean, flags, &SK, &mask, S1_opt, S2_opt,
+                      scratch, (size_t)SK_NOALLOC_SCRATCH_BYTES, (cudaStream_t)stream);
 }
 
 int sk_frame_multi(uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t nlev,
@@ -646,6 +701,7 @@ const char* sk_strerror(int code) {
         case SK_ERR_N: return "receiver count N must be in [1, E]";
         case SK_ERR_PARAM: return "n_sigma and sk_mean must be finite, n_sigma >= 0";
         case SK_ERR_WORKSPACE: return "workspace is NULL, misaligned or smaller than sk_frame_workspace_bytes()";
+        case SK_ERR_SCRATCH: return "sk_frame_noalloc: this shape needs more scratch than the built-in SK_NOALLOC_SCRATCH_BYTES";
         default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown error";
     }
 }
