@@ -121,8 +121,12 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     const uint32_t iters = (M + RPW - 1) / RPW;
     pl.wide = iters <= sk::AccWide2::kMaxSamples;
     pl.chain = iters <= sk::AccChain2::kMaxSamples;
-    // the stream kernel's grid is (slabs, F, B / bpu) and its tensor map has a row of F*E bytes
-    const bool grid_ok = B / bpu <= 65535u && F <= 65535u && (unsigned long long)F * E < (1ull << 32) &&
+    // the stream kernel's grid is (slabs, F, B / bpu) and its tensor map has a row of F*E bytes.  The
+    // coordinates of a TMA box are SIGNED 32-bit: the last box of a row starts below F*E and a ragged
+    // one reaches at most 256 bytes past it, so F*E + 256 <= 2^31 keeps every x (and B*M < 2^31 every
+    // y) non-negative; a wider frame would have its upper boxes read as negative coordinates and
+    // zero-filled.  Such frames take the direct-load kernel.
+    const bool grid_ok = B / bpu <= 65535u && F <= 65535u && (unsigned long long)F * E + 256ull <= (1ull << 31) &&
                          (unsigned long long)B * M < (1ull << 31);
     pl.chunk = (pl.vec && grid_ok && pl.L >= 4) ? chunk_rows(M, pl.L) : 0u;
     if (pl.chunk == 0u && pl.vec && grid_ok && g_force_lanes.load(std::memory_order_relaxed) == 0) {

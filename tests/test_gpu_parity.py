@@ -549,6 +549,15 @@ def test_argument_errors(sk):
         sk.sk_frame(torch.zeros(64, 1, 32, dtype=torch.uint8), 32)          # CPU tensor: no fallback
 
 
+def test_plan_keeps_tma_coordinates_non_negative(sk):
+    """The coordinates of a TMA box are signed 32-bit: a frame whose rows are 2^31 bytes or longer
+    (F*E, still a legal shape) must not be given to the stream kernel, whose upper boxes would come
+    back zero-filled; one just below that still is.  (Plan only: such a frame is >= 64 GiB.)"""
+    assert sk.sk_debug_get_plan(32, 2047, 1 << 20, 32)[2] == 32        # F*E + 256 <= 2^31: TMA stream kernel
+    assert sk.sk_debug_get_plan(32, 2048, 1 << 20, 32)[2] == 0         # F*E = 2^31: direct-load kernel
+    assert sk.sk_debug_get_plan(32, 4095, 1 << 20, 32)[2] == 0
+
+
 def test_host_entry_point(sk, oracle):
     cfg = sk_synth.config(0)
     host = sk_synth.make_frame(cfg).pin_memory()
