@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling", "fig5", "fig6"],
+    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling", "fig5", "fig6", "firstpass"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
@@ -461,6 +461,76 @@ def run_aux(args):
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
+def run_firstpass(args):
+    """--op firstpass: what in-place excision costs the FIRST time a frame is excised.  The headline
+    --zero lines replay frames that earlier steps already excised (the same bytes are rewritten); here
+    every timed frame is fresh: the working copies are restored from masters outside the timed region,
+    then one CUDA graph of one sk_frame call per frame runs inside a CUDA-event pair.  Three cases on
+    the same frames: no excision, the workload's own flags, and every cell flagged (the flag centre moved
+    far away) — the worst case for the fused finalizer, which excises a whole cell with one warp."""
+    import statistics
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = workload(args.workload)
+    l2 = 126 * 1024 * 1024
+    nbuf = max(4, -(-4 * l2 // cfg.nbytes))
+    nbuf = max(2, min(nbuf, int(torch.cuda.mem_get_info()[0] * 0.4) // cfg.nbytes))
+    masters = [sk_synth.make_frame(cfg, device=dev, frame=fid) for fid in frame_ids(0, nbuf)]
+    work = [m.clone() for m in masters]
+    sk_mean = null_mean(sk, sk_synth, cfg, dev)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, stream.cuda_stream)
+        out = sk.sk_frame(work[0], cfg.M, n_sigma=5.0, sk_mean=sk_mean, workspace=ws, stream=stream)
+    torch.cuda.synchronize()
+    n0 = sk.sk_launch_count()
+    rows = []
+    reps = max(args.steps, 5)
+    for name, zero, centre in (("no excision", False, sk_mean), ("excision, the workload's own flags", True, sk_mean),
+                               ("excision, every cell flagged", True, sk_mean + 10.0)):
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for i in range(nbuf):                 # the first call waits for everything before it (the restore)
+                sk.sk_frame(work[i], cfg.M, n_sigma=5.0, sk_mean=centre, zero_flagged=zero, out=out, workspace=ws,
+                            stream=stream, inputs_ready=i > 0)
+        times, flagged = [], 0.0
+        for r in range(reps + 2):
+            with torch.cuda.stream(stream):
+                for w, m in zip(work, masters):
+                    w.copy_(m)                    # fresh bytes: outside the timed region
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                e0.record(stream)
+                graph.replay()
+                e1.record(stream)
+            torch.cuda.synchronize()
+            if r >= 2:
+                times.append(e0.elapsed_time(e1) / nbuf)
+            flagged = float(out.mask.float().mean().item())
+        ms = statistics.median(times)
+        excised = sum(int((w != m).any(dim=2).sum().item()) for w, m in zip(work[-1:], masters[-1:])) if zero else 0
+        rows.append({"case": name, "ms_per_frame": ms, "read_gbs": cfg.nbytes / ms / 1e6,
+                     "flagged_fraction_last_frame": flagged, "rows_changed_last_frame": excised,
+                     "bytes_excised_per_frame": int(round(flagged * cfg.nbytes)) if zero else 0})
+    base = rows[0]["ms_per_frame"]
+    for r in rows[1:]:
+        extra = (r["ms_per_frame"] - base) * 1e-3
+        r["extra_us_per_frame"] = extra * 1e6
+        r["excision_write_gbs"] = r["bytes_excised_per_frame"] / extra / 1e9 if extra > 0 and r["bytes_excised_per_frame"] else None
+    print(json.dumps({
+        "op": "firstpass", "metric": "ms_per_frame", "unit": "ms", "higher_is_better": False, "n_gpus": 1,
+        "steps": reps, "warmup": 2, "data": "synthetic", "dtype": "u8->u32/f64",
+        "config": {"workload": cfg.name, "E": cfg.E, "F": cfg.F, "T": cfg.T, "M": cfg.M, "frame_bytes": cfg.nbytes,
+                   "frames": nbuf, "launch": "one CUDA graph of one sk_frame call per frame, SK_FRAME_INPUTS_READY after the "
+                   "first; working copies restored from masters before every replay; median of %d replays" % reps},
+        "cases": rows, "value": rows[1]["ms_per_frame"], "ms_per_step": rows[1]["ms_per_frame"],
+        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+
+
 def null_mean(sk, sk_synth, cfg, dev, M=None):
     """The flag centre the paper's way: mean SK of an RFI-free simulation with the
     workload's per-input sigmas (the 4-bit null mean is not 1: App. B)."""
@@ -635,6 +705,8 @@ def main():
         return run_fig5(args)
     if args.op == "fig6":
         return run_fig6(args)
+    if args.op == "firstpass":
+        return run_firstpass(args)
     if args.op != "frame":
         return run_aux(args)
 
@@ -679,11 +751,17 @@ def main():
         out = sk.sk_frame(bufs[0], cfg.M, n_sigma=n_sigma, sk_mean=sk_mean, workspace=ws, stream=stream)
     torch.cuda.synchronize()
 
-    # every frame is resident and complete before the timed region starts, and no step writes
-    # another step's frame, so the SK_FRAME_INPUTS_READY promise holds (include/sk_b200.h)
+    # Every frame is resident and complete before the timed region starts.  Without --zero no step
+    # writes any frame, so the SK_FRAME_INPUTS_READY promise (include/sk_b200.h) holds for every step.
+    # With --zero every step excises its own frame and the frames recur every nbuf steps: step
+    # i + nbuf reads what step i wrote.  The promise covers only what was written before the last call
+    # made WITHOUT the flag, so the first step of every pass over the ring (i % nbuf == 0) is made
+    # without it: that kernel waits for all earlier ones (the previous pass's excisions included)
+    # before its first read, and the nbuf - 1 steps after it read frames last written before it.
     def step(i):
+        ready = not args.serialize and not (args.zero and i % nbuf == 0)
         sk.sk_frame(bufs[i % nbuf], cfg.M, n_sigma=n_sigma, sk_mean=sk_mean, zero_flagged=args.zero,
-                    out=out, workspace=ws, stream=stream, inputs_ready=not args.serialize)
+                    out=out, workspace=ws, stream=stream, inputs_ready=ready)
 
     def barrier():
         if world > 1:

@@ -229,11 +229,13 @@ int sk_version(void);
 unsigned long long sk_launch_count(void);
 
 /* Tests and A/B timing only: override the kernel choice of the fused path for the whole process.
- * path = SK_PLAN_AUTO (default) or SK_PLAN_LDG (direct-load kernel instead of the TMA stream
- * kernel); lanes = 0 (automatic) or 1, 2, 4, 8, 16: slab width 16*lanes inputs, if not wider than
+ * path = SK_PLAN_AUTO (default), SK_PLAN_LDG (direct-load kernel instead of the TMA stream
+ * kernel) or SK_PLAN_NO_TMAP; lanes = 0 (automatic) or 1, 2, 4, 8, 16: slab width 16*lanes inputs, if not wider than
  * a row.  Results do not depend on either. */
 #define SK_PLAN_AUTO 0
 #define SK_PLAN_LDG  1
+#define SK_PLAN_NO_TMAP 2   /* plan as usual, but behave as if the driver had refused to encode the tensor
+                             * map: exercises the fall-back to the direct-load kernels (identical results) */
 void sk_debug_set_plan(int path, int lanes);
 
 /* Tests and bench reporting only: the launch plan sk_frame / sk_frame_multi would use for this

@@ -21,7 +21,7 @@ SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes",
 
 # bits of sk_frame's `flags` (include/sk_b200.h)
 SK_FRAME_ZERO_FLAGGED, SK_FRAME_INPUTS_READY, SK_FRAME_EQ13 = 1, 2, 4
-SK_PLAN_AUTO, SK_PLAN_LDG = 0, 1
+SK_PLAN_AUTO, SK_PLAN_LDG, SK_PLAN_NO_TMAP = 0, 1, 2
 
 _lib = None
 

@@ -166,18 +166,25 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     return pl;
 }
 
-template <class Acc2>
-void launch_vec_L(int L, const sk::FrameParams& p, cudaStream_t st) {
+template <class Acc2, bool EXC>
+void launch_vec_LX(int L, const sk::FrameParams& p, cudaStream_t st) {
     const unsigned grid = (p.nunits + sk::kWarpsPerCta - 1) / sk::kWarpsPerCta;
     const unsigned block = sk::kWarpsPerCta * 32;
     switch (L) {
-        case 16: sk::sk_frame_kernel<16, Acc2><<<grid, block, 0, st>>>(p); break;
-        case 8:  sk::sk_frame_kernel<8, Acc2><<<grid, block, 0, st>>>(p); break;
-        case 4:  sk::sk_frame_kernel<4, Acc2><<<grid, block, 0, st>>>(p); break;
-        case 2:  sk::sk_frame_kernel<2, Acc2><<<grid, block, 0, st>>>(p); break;
-        default: sk::sk_frame_kernel<1, Acc2><<<grid, block, 0, st>>>(p); break;
+        case 16: sk::sk_frame_kernel<16, Acc2, EXC><<<grid, block, 0, st>>>(p); break;
+        case 8:  sk::sk_frame_kernel<8, Acc2, EXC><<<grid, block, 0, st>>>(p); break;
+        case 4:  sk::sk_frame_kernel<4, Acc2, EXC><<<grid, block, 0, st>>>(p); break;
+        case 2:  sk::sk_frame_kernel<2, Acc2, EXC><<<grid, block, 0, st>>>(p); break;
+        default: sk::sk_frame_kernel<1, Acc2, EXC><<<grid, block, 0, st>>>(p); break;
     }
     ++g_launches;
+}
+
+// A launch that excises in place reads `data` without .nc (see sk_frame_kernel).
+template <class Acc2>
+void launch_vec_L(int L, const sk::FrameParams& p, cudaStream_t st) {
+    if (p.excise) launch_vec_LX<Acc2, true>(L, p, st);
+    else          launch_vec_LX<Acc2, false>(L, p, st);
 }
 
 // ---- TMA path ---------------------------------------------------------------------------
@@ -268,6 +275,10 @@ int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, bool chun
     }
 }
 
+// launch_stream could not build the tensor map for this pointer / shape (nothing was launched): the
+// callers fall back to the direct-load kernels, whose results are identical.  Never returned to a user.
+constexpr int kEncodeFailed = -1000;
+
 int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     CUtensorMap tmap;
     const uint32_t W = 16u * pl.L;
@@ -278,7 +289,7 @@ int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     const CUresult r = encode_tiled()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(p.data), gdim,
                                       gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    if (r != CUDA_SUCCESS || g_force_path.load(std::memory_order_relaxed) == SK_PLAN_NO_TMAP) return kEncodeFailed;
     const bool chunked = pl.chunk != p.M;
     const uint32_t zblocks = p.B / pl.bpu;
     int rc;
@@ -305,16 +316,23 @@ int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
     if (pl.vec) {
         p.slabs = pl.slabs;
         p.nunits = cells * pl.slabs;
+        int rc = kEncodeFailed;                                    // "no stream kernel": also when it is not wanted
         if (stream_wanted(pl)) {
             p.chunk = pl.chunk;
             p.bpu = pl.bpu;
             p.tpb = pl.ragged_tpb;
             p.unit_tiles = pl.ragged_tpb ? pl.ragged_tpb * pl.bpu : p.M * pl.bpu / (sk::kTileBytes / (16u * pl.L));
-            const int rc = launch_stream(pl, p, st);
-            if (rc != SK_OK) return rc;
-        } else if (pl.chain) launch_vec_L<sk::AccChain2>(pl.L, p, st);
-        else if (pl.wide)  launch_vec_L<sk::AccWide2>(pl.L, p, st);
-        else               launch_vec_L<sk::AccPlain2>(pl.L, p, st);
+            rc = launch_stream(pl, p, st);
+            if (rc != SK_OK && rc != kEncodeFailed) return rc;
+            if (rc == kEncodeFailed && p.nlev > 1) return rc;      // frame_impl takes one pass per length instead
+        }
+        if (rc == kEncodeFailed) {
+            // the direct-load kernel at this slab width: one cell per unit, accumulators by block length
+            const uint32_t iters = (p.M + 32u / pl.L - 1) / (32u / pl.L);
+            if (iters <= sk::AccChain2::kMaxSamples)     launch_vec_L<sk::AccChain2>(pl.L, p, st);
+            else if (iters <= sk::AccWide2::kMaxSamples) launch_vec_L<sk::AccWide2>(pl.L, p, st);
+            else                                         launch_vec_L<sk::AccPlain2>(pl.L, p, st);
+        }
     } else {
         sk::sk_cell_kernel_scalar<<<cells, sk::kScalarThreads, 0, st>>>(p);
         ++g_launches;
@@ -395,7 +413,10 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
             ws += level_bytes(cells, slabs_max);
         }
     }
-    if (one_launch) return launch_cells(pl, p, st);
+    if (one_launch) {
+        const int rc = launch_cells(pl, p, st);
+        if (rc != kEncodeFailed) return rc;                        // only with nlev > 1: no tensor map, take the passes below
+    }
     // several lengths without the stream kernel: one pass of the fused path per length, then the
     // excision of every flagged cell of every length (all lengths see the data before excision)
     for (uint32_t l = 0; l < nlev; ++l) {
@@ -766,7 +787,7 @@ int sk_debug_pipe_rate(int mode, uint32_t warps_per_sm, uint32_t* io, unsigned l
 }
 
 void sk_debug_set_plan(int path, int lanes) {
-    g_force_path.store(path == SK_PLAN_LDG ? SK_PLAN_LDG : SK_PLAN_AUTO);
+    g_force_path.store((path == SK_PLAN_LDG || path == SK_PLAN_NO_TMAP) ? path : SK_PLAN_AUTO);
     g_force_lanes.store((lanes >= 1 && lanes <= 16 && (lanes & (lanes - 1)) == 0) ? lanes : 0);
 }
 

@@ -20,6 +20,15 @@ __device__ __forceinline__ uint4 ldg_stream(const uint8_t* p) {
     return r;
 }
 
+// The same load without .nc, for a kernel that also WRITES the buffer it reads (in-place excision):
+// PTX allows ld.global.nc only on memory that stays read-only for the kernel's whole lifetime.
+__device__ __forceinline__ uint4 ldg_stream_rw(const uint8_t* p) {
+    uint4 r;
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
 // Scheduling fence for a batch of loads: every register of the batch passes through one empty
 // volatile asm, so all loads of the batch are issued before the first sample is unpacked
 // (keeps kUnroll 128-bit loads in flight per lane instead of one).

@@ -296,9 +296,12 @@ __device__ __forceinline__ void publish_and_finalize(const FrameParams& p, int l
 }
 
 // --------------------------------------------------------------------------- fused a1..a7
-// Direct-load fallback of the stream kernel (sk_tma.cuh): the same unit decomposition, 128-bit
-// ld.global.nc loads, one integration length.  Acc2 = AccChain2 / AccWide2 / AccPlain2 by block length.
-template <int L, class Acc2>
+// Direct-load fallback of the stream kernel (sk_tma.cuh): the same unit decomposition, 128-bit global
+// loads, one integration length.  Acc2 = AccChain2 / AccWide2 / AccPlain2 by block length.
+// EXC = the launch excises flagged cells in place (p.excise != nullptr): the data is then read with
+// plain ld.global instead of ld.global.nc, because another warp of this grid may be overwriting a
+// neighbouring cell of the same 32-byte sector while this one loads (E = 16).
+template <int L, class Acc2, bool EXC>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, kMinCtasPerSm)
 sk_frame_kernel(const FrameParams p) {
     constexpr int RPW = 32 / L;
@@ -330,14 +333,14 @@ sk_frame_kernel(const FrameParams p) {
             for (; i + kUnroll <= mine; i += kUnroll) {
                 uint4 v[kUnroll];
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) v[u] = ldg_stream(q + (size_t)u * step);
+                for (int u = 0; u < kUnroll; ++u) v[u] = EXC ? ldg_stream_rw(q + (size_t)u * step) : ldg_stream(q + (size_t)u * step);
                 q += (size_t)kUnroll * step;
                 loads_issued(v);
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) accumulate16(acc, v[u], kc);
             }
             for (; i < mine; ++i) {
-                const uint4 v = ldg_stream(q);
+                const uint4 v = EXC ? ldg_stream_rw(q) : ldg_stream(q);
                 q += step;
                 accumulate16(acc, v, kc);
             }

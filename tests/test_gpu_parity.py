@@ -152,15 +152,25 @@ def test_config1_full_frame(sk, oracle, vector_path):
     """BASELINE.json config 1, full size (96 MiB, 192 cells), in the launch configuration bench.py
     times (default arguments, no sums requested) plus a second run with sums."""
     cfg = sk_synth.config(1)
+    # the flag is centred on the simulated null mean (PAPER.md:284), as bench.py does: on 4-bit data the
+    # null mean is ~0.914, and around 1.0 every cell of this RFI-free frame would be flagged (a mask test
+    # that cannot fail); around the null mean the mask is clean because the frame is
+    sk_mean = _oracle_null_mean(oracle, cfg)
     data = sk_synth.make_frame(cfg, device="cuda")
-    out = sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
+    out = sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=sk_mean)
     torch.cuda.synchronize()
     host = data.cpu()
-    ref = oracle.frame(host.numpy(), cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
+    ref = oracle.frame(host.numpy(), cfg.M, n_sigma=cfg.n_sigma, sk_mean=sk_mean)
     assert_sk_close(out.SK.cpu().numpy(), ref["SK"])
     np.testing.assert_array_equal(out.mask.cpu().numpy(), ref["mask"])
+    assert ref["mask"].mean() < 0.05                       # 3 sigma on 192 null cells: a handful at most
+    # and around 1.0 (Eq. 15's un-digitised centre) the 4-bit offset flags every cell, on both sides
+    off = sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0)
+    off_ref = oracle.flag(ref["SK"].astype(np.float32), cfg.M, cfg.E, cfg.n_sigma, 1.0)
+    np.testing.assert_array_equal(off.mask.cpu().numpy(), off_ref)
+    assert off_ref.all()
     # the launch configuration bench.py times: back-to-back calls with SK_FRAME_INPUTS_READY
-    piped = [sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=1.0, inputs_ready=True) for _ in range(4)]
+    piped = [sk.sk_frame(data, cfg.M, n_sigma=cfg.n_sigma, sk_mean=sk_mean, inputs_ready=True) for _ in range(4)]
     torch.cuda.synchronize()
     for o in piped:
         assert torch.equal(o.SK.view(torch.int32), out.SK.view(torch.int32)) and torch.equal(o.mask, out.mask)
@@ -393,6 +403,7 @@ def test_pipelined_frames_inputs_ready(sk, oracle):
         assert int(ws.abs().sum().item()) == 0
     # excision between pipelined frames (the finalizer of a flagged cell overwrites it)
     work = [d.clone() for d in frames[:4]]
+    torch.cuda.synchronize()            # the promise: nothing enqueued since the last synchronisation writes `data`
     outs = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, workspace=ws, zero_flagged=True, inputs_ready=True)
             for d in work]
     torch.cuda.synchronize()
@@ -625,6 +636,40 @@ def test_frame_multi_excision_is_the_union(sk, oracle, vector_path):
     np.testing.assert_array_equal(d.cpu().numpy(), expect)
 
 
+def test_tensor_map_refusal_falls_back_to_direct_loads(sk, oracle):
+    """If the driver refuses to encode the tensor map, sk_frame and sk_frame_multi must not fail:
+    the direct-load kernels (one pass per length for sk_frame_multi) give the same results.
+    SK_PLAN_NO_TMAP makes the library behave as after such a refusal."""
+    T, F, E, M, nlev = 4096, 2, 2048, 128, 3
+    data = sk_synth.make_frame(sk_synth.config(2).with_(T=T, F=F, E=E, M=M))
+    means = [0.91, 0.912, 0.913]
+    d0, d1 = data.cuda(), data.cuda()
+    want1 = sk.sk_frame(d0.clone(), 256, n_sigma=4.0, sk_mean=0.913, want_sums=True, zero_flagged=True)
+    want = sk.sk_frame_multi(d0, M, nlev, n_sigma=4.0, sk_means=means, zero_flagged=True)
+    ragged = sk_synth.random_bytes(3000, 1, 512, seed=77).cuda()      # M = 1000: the ragged stream kernel
+    want_r = sk.sk_frame(ragged, 1000, sk_mean=0.4)
+    n0 = sk.sk_launch_count()
+    sk.sk_debug_set_plan(sk.SK_PLAN_NO_TMAP, 0)
+    assert sk.sk_debug_get_plan(T, F, E, M, nlev=nlev)[2] != 0        # the plan still asks for the stream kernel
+    got1 = sk.sk_frame(d1.clone(), 256, n_sigma=4.0, sk_mean=0.913, want_sums=True, zero_flagged=True)
+    got = sk.sk_frame_multi(d1, M, nlev, n_sigma=4.0, sk_means=means, zero_flagged=True)
+    got_r = sk.sk_frame(ragged, 1000, sk_mean=0.4)
+    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+    torch.cuda.synchronize()
+    assert sk.sk_launch_count() - n0 == 1 + (nlev + nlev) + 1       # fused; one pass and one excision per length; fused
+    assert torch.equal(got1.SK.view(torch.int32), want1.SK.view(torch.int32)) and torch.equal(got1.mask, want1.mask)
+    assert torch.equal(got1.S1.view(torch.int32), want1.S1.view(torch.int32))
+    assert torch.equal(got1.S2.view(torch.int32), want1.S2.view(torch.int32))
+    assert torch.equal(got_r.SK.view(torch.int32), want_r.SK.view(torch.int32)) and torch.equal(got_r.mask, want_r.mask)
+    for l in range(nlev):
+        assert torch.equal(got.SK[l].view(torch.int32), want.SK[l].view(torch.int32)), l
+        assert torch.equal(got.mask[l], want.mask[l]), l
+        ref = oracle.frame(data.numpy(), M << l, n_sigma=4.0, sk_mean=means[l])
+        assert_sk_close(got.SK[l].cpu().numpy(), ref["SK"])
+        np.testing.assert_array_equal(got.mask[l].cpu().numpy(), ref["mask"])
+    assert torch.equal(d0, d1)                                         # the same bytes were excised
+
+
 def test_frame_multi_argument_errors(sk):
     d = torch.zeros(96, 1, 32, dtype=torch.uint8, device="cuda")
     with pytest.raises(sk.SKError):
@@ -693,6 +738,7 @@ def test_ragged_blocks_pipelined_with_excision(sk, oracle):
         fr[M:2 * M, 0, :] = 0x88
     work = [fr.cuda() for fr in frames]
     ws = sk.workspace_for(T, F, E, M, work[0].device, 3003)
+    torch.cuda.synchronize()            # uploads and workspace fill are complete: the promise holds
     outs = [sk.sk_frame(d, M, n_sigma=2.0, sk_mean=0.4, zero_flagged=True, inputs_ready=True, workspace=ws) for d in work]
     torch.cuda.synchronize()
     assert int(ws.abs().sum().item()) == 0
@@ -731,6 +777,7 @@ def test_randomised_shapes_and_flags(sk, oracle):
         sk.sk_debug_set_plan(path, lanes)
         ref = oracle.frame(data.numpy(), M, n_sigma=ns, sk_mean=sk_mean, zero_flagged=zero, **kw)
         d = data.cuda()
+        torch.cuda.synchronize()
         out = sk.sk_frame(d, M, n_sigma=ns, sk_mean=sk_mean, zero_flagged=zero, want_sums=sums, inputs_ready=ready, **kw)
         torch.cuda.synchronize()
         case = (it, T, F, E, M, sorted(kw), zero, sums, ready, path, lanes)
