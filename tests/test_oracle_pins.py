@@ -494,6 +494,36 @@ def test_sim_digitised_layout_and_pmf(oracle):
     assert abs(np.sqrt((pmf152 * np.arange(-7, 8) ** 2).sum()) - 1.52) < 0.04
 
 
+def test_digitiser_thresholds_exact():
+    """sk_synth.digitiser_thresholds is App. B's input model (components rounded to the
+    nearest level and bounded to [-7, 7]) and feeds BOTH simulators, so neither parity test can see a
+    mistake in it.  Pin it on its own, exactly: thr[e][k] = floor(2^32 Phi((k - 6.5) / sigma_e)), Phi from
+    math.erfc (not the torch routine the table is built with).  An edge off by one level (k - 7.5,
+    k - 5.5) moves a threshold by ~1e8; the comparison allows 1 count for the last bit of Phi."""
+    import sk_synth
+    from math import erfc, floor, sqrt
+    sig = [0.7, 1.0, 1.52, 2.5, 3.5, 9.0]
+    thr = sk_synth.digitiser_thresholds(sig).numpy().astype(np.int64)
+    assert thr.shape == (len(sig), 14)
+    exact = 0
+    for e, s_ in enumerate(sig):
+        for k in range(14):
+            want = floor(4294967296.0 * 0.5 * erfc(-(k - 6.5) / s_ / sqrt(2.0)))
+            assert abs(int(thr[e, k]) - want) <= 1, (s_, k, int(thr[e, k]), want)
+            exact += int(thr[e, k]) == want
+        assert (np.diff(thr[e]) >= 0).all() and (np.diff(thr[e, 3:11]) > 0).all()   # ascending (the tails saturate for a small sigma)
+        assert (thr[e] + thr[e][::-1] - 4294967296 >= -2).all() and (thr[e] + thr[e][::-1] - 4294967296 <= 0).all()   # symmetric levels
+    assert exact >= len(sig) * 14 - 2
+    # sigma = 1: a textbook value, Phi(0.5) = 0.6914624612740131 -> level 0 ends at floor(2^32 * 0.69146...)
+    assert abs(int(thr[1, 7]) - 2969808657) <= 1 and abs(int(thr[1, 6]) - (4294967296 - 2969808657)) <= 1
+    # the clamps: sigma -> 0 puts everything on level 0 (thresholds 0 below the centre, 2^32 - 1 above, never
+    # 2^32, which would not fit); a huge sigma gives the two outer levels half the mass each
+    tiny = sk_synth.digitiser_thresholds([1e-6]).numpy().astype(np.int64)[0]
+    assert (tiny[:7] == 0).all() and (tiny[7:] == 4294967295).all()
+    huge = sk_synth.digitiser_thresholds([1e9]).numpy().astype(np.int64)[0]
+    assert (np.abs(huge - 2147483648) < 64).all() and (np.diff(huge) >= 0).all()
+
+
 def test_app_b_mean_offset_constant_variance_converges(oracle):
     """PAPER.md:282-284 on the simulator's data (sigma = 1.52): the mean of SK~ is offset from 1 by
     a constant that does not depend on N and equals the model's E[p^2]/E[p]^2 - 1; the variance
