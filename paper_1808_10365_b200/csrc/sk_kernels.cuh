@@ -276,8 +276,11 @@ __device__ __forceinline__ uint32_t finalize_cell(const FrameParams& p, int l, u
 // Fused kernels: publish the unit's partial of cell (b, f) at length M << l; the last unit of the
 // cell to arrive finalizes it and, if asked to, excises it (every unit has finished reading the
 // cell by then).
-__device__ __forceinline__ void publish_and_finalize(const FrameParams& p, int l, uint32_t b, uint32_t f,
-                                                     uint32_t slab, int lane, double part) {
+// DEFER: do not excise here; return 1 (on every lane) when the cell is flagged and has to be excised,
+// so that the caller can do it its own way (the stream kernel: TMA bulk stores).  Otherwise returns 0.
+template <bool DEFER = false>
+__device__ __forceinline__ uint32_t publish_and_finalize(const FrameParams& p, int l, uint32_t b, uint32_t f,
+                                                         uint32_t slab, int lane, double part) {
     const uint32_t cell = b * p.F + f;
     double* slots = p.lev[l].partial + (size_t)cell * p.slabs;
     uint32_t last = 0;
@@ -286,13 +289,17 @@ __device__ __forceinline__ void publish_and_finalize(const FrameParams& p, int l
         last = (atomicAdd(p.lev[l].counter + cell, 1u) == p.slabs - 1u);
     }
     last = __shfl_sync(0xffffffffu, last, 0);
-    if (!last) return;
+    if (!last) return 0u;
     const uint32_t flagged = finalize_cell<true>(p, l, cell, lane, slots);
     __syncwarp();
     // leave the workspace all-zero: partials and counter (header contract)
     for (uint32_t s = lane; s < p.slabs; s += 32) slots[s] = 0.0;
     if (lane == 0) p.lev[l].counter[cell] = 0u;
-    if (flagged && p.excise) excise_cell<true>(p, b * (p.M << l), p.M << l, f, lane, 32);
+    if (flagged && p.excise) {
+        if (DEFER) return 1u;
+        excise_cell<true>(p, b * (p.M << l), p.M << l, f, lane, 32);
+    }
+    return 0u;
 }
 
 // --------------------------------------------------------------------------- fused a1..a7

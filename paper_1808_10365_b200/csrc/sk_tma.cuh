@@ -67,6 +67,45 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
+// 2-D tiled TMA store of one box from shared memory (bulk async-group completion).
+__device__ __forceinline__ void tma_store_tile(const CUtensorMap* tmap, uint32_t x, uint32_t y, uint32_t src) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(tmap), "r"(x), "r"(y), "r"(src) : "memory");
+}
+
+// a8 for the stream kernel ("excision"): every byte of a flagged cell becomes 0x88.  The
+// cell is rows [row0, row0 + rows) of frequency f, all E inputs; the whole warp calls.  A finalizer
+// excises the WHOLE cell (512 KiB on config 1) while it holds an SM slot, so how it writes decides the
+// kernel's tail when many cells are flagged.  When the warp's TMA ring is idle (ring_free: the unit's
+// last tile has been consumed) and the cell is a whole number of boxes (E % W == 0; rows % R == 0 holds
+// for this kernel), one ring slot is filled with 0x88 and the cell is written as rows/R x E/W bulk tensor
+// stores of 8 KiB through the same tensor map the loads use: 64 instructions per config-1 cell instead
+// of 1024 128-bit stores with their address arithmetic.  Otherwise (a cell that completes in the middle
+// of a unit, a ragged last slab) the lanes store the bytes themselves.
+template <int L>
+__device__ __forceinline__ void excise_cell_stream(const CUtensorMap* tmap, const FrameParams& p, uint32_t ring,
+                                                   bool ring_free, uint32_t row0, uint32_t rows, uint32_t f, int lane) {
+    constexpr uint32_t W = 16 * L, R = kTileBytes / W;
+    if (!ring_free || p.E % W != 0u || rows % R != 0u) {
+        excise_cell<true>(p, row0, rows, f, (uint32_t)lane, 32u);
+        return;
+    }
+#pragma unroll
+    for (int i = 0; i < kTileBytes / (32 * 16); ++i)
+        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(ring + (uint32_t)(i * 32 + lane) * 16u), "r"(0x88888888u)
+                     : "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the fill, visible to the TMA engine
+    __syncwarp();
+    const uint32_t nx = p.E / W, n = nx * (rows / R);
+    for (uint32_t k = (uint32_t)lane; k < n; k += 32u) {
+        const uint32_t iy = k / nx, ix = k - iy * nx;
+        tma_store_tile(tmap, f * p.E + ix * W, row0 + iy * R, ring);
+    }
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");         // written, not only read: the slot may be reused or freed
+    __syncwarp();
+}
+
 // 128 registers = 13 resident warps.  Several integration lengths keep 16 more running sums per
 // length and lane (touched once per M-row block) in registers: a higher limit, fewer resident warps.
 // Measured on config 2 with 4 lengths (us per frame; 210 for one length): all in registers,
@@ -197,17 +236,21 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
                 for (int i = 0; i < kOwn; ++i) { o1[i] = S1[i]; o2[i] = S2[i]; }
             }
         }
-        if (p.lev[0].SK)
-            publish_and_finalize(p, 0, b0, f, slab, lane,
-                                 unit_partial<L>(p, (double)p.M, active, owner, e_first, S1, S2));
+        const bool ring_free = g + 1u == total;    // the unit's last tile: nothing is in flight into the ring any more
+        if (p.lev[0].SK) {
+            if (publish_and_finalize<true>(p, 0, b0, f, slab, lane,
+                                           unit_partial<L>(p, (double)p.M, active, owner, e_first, S1, S2)))
+                excise_cell_stream<L>(&tmap, p, ring, ring_free, b0 * p.M, p.M, f, lane);
+        }
         ++blk;
 #pragma unroll
         for (int l = 1; l < NLEV; ++l) {
 #pragma unroll
             for (int i = 0; i < kOwn; ++i) { up1[l - 1][i] += S1[i]; up2[l - 1][i] += S2[i]; }
             if ((blk & ((1u << l) - 1u)) == 0u) {  // the last block of a cell of length M << l
-                publish_and_finalize(p, l, (b0 >> l), f, slab, lane,
-                                     unit_partial<L>(p, (double)(p.M << l), active, owner, e_first, up1[l - 1], up2[l - 1]));
+                if (publish_and_finalize<true>(p, l, (b0 >> l), f, slab, lane,
+                                               unit_partial<L>(p, (double)(p.M << l), active, owner, e_first, up1[l - 1], up2[l - 1])))
+                    excise_cell_stream<L>(&tmap, p, ring, ring_free, (b0 >> l) * (p.M << l), p.M << l, f, lane);
 #pragma unroll
                 for (int i = 0; i < kOwn; ++i) up1[l - 1][i] = up2[l - 1][i] = 0;
             }
