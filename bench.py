@@ -43,13 +43,13 @@ def parse():
     ap.add_argument("--serialize", action="store_true",
                     help="do not pass SK_FRAME_INPUTS_READY: each frame waits for the previous one to finish")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 20)")
-    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling", "fig5", "fig6", "firstpass"],
+    ap.add_argument("--op", default="frame", choices=["frame", "multi", "rebin", "single", "sim", "cm", "ceiling", "memonly", "eager", "fig5", "fig6", "firstpass"],
                     help="frame = the fused hot path (the contract's line); rebin / single = the SURVEY 8(f) "
                          "outputs next to it (sk_rebin_sums factor 2, sk_single), timed on config-4-sized sums")
     ap.add_argument("--path", default="auto", choices=["auto", "ldg"],
-                    help="A/B timing: ldg = the direct-load kernel instead of the TMA stream kernel (sk_debug_set_plan)")
+                    help="A/B timing: ldg = the direct-load kernel instead of the TMA stream kernel (the SK_FRAME_PLAN_LDG bit of the call's flags)")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 4, 8, 16],
-                    help="A/B timing: force a slab width of 16*lanes inputs (sk_debug_set_plan); 0 = automatic")
+                    help="A/B timing: force a slab width of 16*lanes inputs (SK_FRAME_PLAN_LANES in the call's flags); 0 = automatic")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -110,14 +110,15 @@ def issue_roofline(name, samples_per_launch, achieved_samples_per_s):
 
 
 def sm_ceiling(sk, torch, dev, sm_mhz, sm_max_mhz, achieved_samples_per_s, warps=12):
-    """The SM-side ceiling of the hot loop, MEASURED in this run (sk_debug_loop_ceiling: the kernel's
+    """The SM-side ceiling of the hot loop, MEASURED in this run (skb_loop_ceiling of the bench library: the kernel's
     a1-a3 loop on a fixed shared-memory tile, no memory traffic, `warps` warps per SM as in the kernel):
     sub-partition cycles per 32 samples -> samples/s at the SM clock the timed region ran at."""
-    cyc = sk.sk_debug_loop_ceiling(warps, 100, dev)
+    from paper_1808_10365_b200 import benchlib
+    cyc = benchlib.loop_ceiling(warps, 100, dev)
     subp = 4 * torch.cuda.get_device_properties(dev).multi_processor_count
     out = {"subpartition_cycles_per_32_samples": cyc, "warps_per_sm": warps, "subpartitions": subp,
            "samples_per_s_at_sm_max": subp * 32 * (sm_max_mhz or 1965) * 1e6 / cyc,
-           "what": "sk_debug_loop_ceiling: the stream kernel's tile loop alone (no HBM, TMA, barrier or epilogue)"}
+           "what": "skb_loop_ceiling (libsk_b200_bench.so): the stream kernel's tile loop alone (no HBM, TMA, barrier or epilogue)"}
     if sm_mhz:
         out["samples_per_s_at_observed_clock"] = subp * 32 * sm_mhz * 1e6 / cyc
         out["frac_at_observed_clock"] = achieved_samples_per_s / out["samples_per_s_at_observed_clock"]
@@ -125,16 +126,19 @@ def sm_ceiling(sk, torch, dev, sm_mhz, sm_max_mhz, achieved_samples_per_s, warps
 
 
 def run_ceiling(args):
-    """--op ceiling: the SM-side ceiling of the hot loop for 4..16 warps per SM."""
+    """--op ceiling: the SM-side ceiling of the hot loop for 4..16 warps per SM, the same loop with one
+    kind of instruction left out (attribution by removal), and the issue rates of its instructions."""
     import torch
-    import paper_1808_10365_b200 as sk
+    from paper_1808_10365_b200 import benchlib
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
-    n0 = sk.sk_launch_count()
-    sk.sk_debug_loop_ceiling(12, 20, dev)
-    pts = [{"warps_per_sm": w, "subpartition_cycles_per_32_samples": sk.sk_debug_loop_ceiling(w, 200, dev)}
+    n0 = benchlib.launch_count()
+    benchlib.loop_ceiling(12, 20, dev)
+    pts = [{"warps_per_sm": w, "subpartition_cycles_per_32_samples": benchlib.loop_ceiling(w, 200, dev)}
            for w in (4, 8, 12, 16)]
-    pipes = {name: sk.sk_debug_pipe_rate(m, 16, dev) for m, name in enumerate(sk.PIPE_MODES)}
+    removal = {name: benchlib.loop_ceiling(12, 200, dev, variant=v) for name, v in benchlib.VARIANTS.items()
+               if name != "memonly"}
+    pipes = {name: benchlib.pipe_rate(m, 16, dev) for m, name in enumerate(benchlib.PIPE_MODES)}
     # the loop alone for ~1.5 s with the NVML record: what the arithmetic draws without any memory traffic
     sampler = ClockSampler(0)
     sampler.start()
@@ -142,7 +146,7 @@ def run_ceiling(args):
     sampler.window = (t_lo, None)
     cyc_long, calls = [], 0
     while time.perf_counter() - t_lo < 1.5:
-        cyc_long.append(sk.sk_debug_loop_ceiling(12, 4000, dev))
+        cyc_long.append(benchlib.loop_ceiling(12, 4000, dev))
         calls += 1
     t_hi = time.perf_counter()
     sampler.window = (t_lo, t_hi)
@@ -157,13 +161,155 @@ def run_ceiling(args):
         "config": {"workload": "the stream kernel's tile loop on a fixed shared-memory tile (no HBM traffic)",
                    "value_is": "sub-partitions x 32 lanes x 1.965 GHz / cycles per 32 samples at 12 warps per SM",
                    "points": pts,
+                   "removal_at_12_warps": removal,
+                   "removal_note": "sub-partition cycles per 32 samples of the same loop with one kind of instruction left "
+                                   "out (sums are then wrong): no_fadd2 = without sub.rn.f32x2, no_prmt = without the four "
+                                   "PRMT per word, no_unpack = without LOP3/SHF/LOP3",
                    "subpartition_cycles_per_warp_instruction": pipes,
                    "pipes_note": "16 warps per SM, 8 independent chains per lane; pairs count two instructions",
                    "loop_for_1.5_s": {"clocks": loop_clocks, "samples_per_s": loop_rate,
                                       "pj_per_sample": (loop_clocks["power_w"] or 0) / loop_rate * 1e12,
                                       "note": "12 warps per SM, back-to-back launches: board power of the arithmetic "
                                               "alone (no HBM traffic), idle power included"}},
-        "gpu_launches": int(sk.sk_launch_count() - n0)}))
+        "gpu_launches": int(benchlib.launch_count() - n0)}))
+
+
+def run_memonly(args):
+    """--op memonly: is memory the limit?  The product's TMA stream kernel (skb_stream of the bench library:
+    same loads, ring, epilogue, finalizer and programmatic dependent launch) on config-1 frames, once with the
+    product's loop body and once with the arithmetic replaced by an XOR of the loaded words, in the headline's
+    steady-state protocol (a CUDA graph of 200 launches replayed for --seconds inside one event pair, after half
+    as long untimed) and in a burst after --cooldown seconds of idle."""
+    import torch
+    import sk_synth
+    from paper_1808_10365_b200 import benchlib
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = workload(args.workload)
+    l2 = 126 * 1024 * 1024
+    nbuf = max(4, -(-5 * l2 // cfg.nbytes))
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=fid) for fid in frame_ids(0, nbuf)]
+    B = cfg.T // cfg.M
+    stream = torch.cuda.Stream(device=dev)
+    SK = torch.empty((B, cfg.F), dtype=torch.float32, device=dev)
+    mask = torch.empty((B, cfg.F), dtype=torch.uint8, device=dev)
+    ws = benchlib.stream_workspace(cfg.T, cfg.F, cfg.E, cfg.M, dev)
+    torch.cuda.synchronize()
+    peak, peak_src = peaks()
+    n0 = benchlib.launch_count()
+    rows = []
+    G = 200
+
+    def barrier():
+        torch.cuda.synchronize()
+
+    for name in ("product", "memonly"):
+        var = benchlib.VARIANTS[name]
+        with torch.cuda.stream(stream):
+            for i in range(5):
+                benchlib.stream(var, bufs[i % nbuf], cfg.M, SK, mask, ws, inputs_ready=True, stream=stream)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for i in range(G):
+                benchlib.stream(var, bufs[i % nbuf], cfg.M, SK, mask, ws, inputs_ready=True, stream=stream)
+        with torch.cuda.stream(stream):
+            graph.replay()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        time.sleep(args.cooldown)
+        ms_b, reps_b, clocks_b = timed_replays(torch, graph, stream, args.burst_seconds or 0.02, 2e-5, G, barrier, sampler)
+        timed_replays(torch, graph, stream, args.seconds / 2, ms_b * 1e-3 / (reps_b * G), G, barrier)
+        ms, reps, clocks = timed_replays(torch, graph, stream, args.seconds, ms_b * 1e-3 / (reps_b * G), G, barrier, sampler)
+        sampler.stop_flag = True
+        per = ms / (reps * G)
+        per_b = ms_b / (reps_b * G)
+        rows.append({"variant": name, "us_per_frame": per * 1e3, "read_gbs": cfg.nbytes / per / 1e6,
+                     "frac_of_peak": cfg.nbytes / per / 1e6 / peak, "clocks": clocks,
+                     "pj_per_byte": (clocks["power_w"] or 0) / (cfg.nbytes / (per * 1e-3)) * 1e12,
+                     "burst": {"us_per_frame": per_b * 1e3, "read_gbs": cfg.nbytes / per_b / 1e6,
+                               "frac_of_peak": cfg.nbytes / per_b / 1e6 / peak, "clocks": clocks_b}})
+    print(json.dumps({
+        "op": "memonly", "metric": "hbm_read_gbs", "value": rows[1]["read_gbs"], "unit": "GB/s", "n_gpus": 1,
+        "steps": G, "warmup": 5, "ms_per_step": rows[1]["us_per_frame"] * 1e-3, "higher_is_better": True,
+        "data": "synthetic", "dtype": "u8",
+        "config": {"workload": cfg.name, "frame_bytes": cfg.nbytes, "frames": nbuf,
+                   "launch": "one CUDA graph of %d skb_stream launches (programmatic dependent launch, inputs ready), "
+                             "replayed for %.2f s inside one CUDA-event pair after %.2f s untimed; burst: %.2f s after "
+                             "%.1f s idle" % (G, args.seconds, args.seconds / 2, args.burst_seconds or 0.02, args.cooldown),
+                   "peak_gbs": peak, "peak_source": peak_src},
+        "variants": rows, "gpu_launches": int(benchlib.launch_count() - n0)}))
+
+
+def run_eager(args):
+    """--op eager: what a caller WITHOUT a CUDA graph gets.  Plain back-to-back sk_frame calls issued from a C
+    loop (skb_frame_loop of the bench library calls the product's own entry point), with and without
+    SK_FRAME_INPUTS_READY, for about --seconds each after half as long untimed; device time from a CUDA-event
+    pair around the loop, host time per call from the loop's own clock."""
+    import torch
+    import paper_1808_10365_b200 as sk
+    import sk_synth
+    from paper_1808_10365_b200 import benchlib
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = workload(args.workload)
+    l2 = 126 * 1024 * 1024
+    nbuf = 10 if cfg.nbytes > l2 else max(4, -(-5 * l2 // cfg.nbytes))
+    nbuf = max(2, min(nbuf, int(torch.cuda.mem_get_info()[0] * 0.8) // cfg.nbytes))
+    bufs = [sk_synth.make_frame(cfg, device=dev, frame=fid) for fid in frame_ids(0, nbuf)]
+    sk_mean = null_mean(sk, sk_synth, cfg, dev)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        ws = sk.workspace_for(cfg.T, cfg.F, cfg.E, cfg.M, dev, stream.cuda_stream)
+        out = sk.sk_frame(bufs[0], cfg.M, n_sigma=5.0, sk_mean=sk_mean, workspace=ws, stream=stream)
+    torch.cuda.synchronize()
+    peak, peak_src = peaks()
+    n0 = sk.sk_launch_count()
+    rows = []
+    for name, flags in (("SK_FRAME_INPUTS_READY", sk.binding.SK_FRAME_INPUTS_READY), ("no flag (each frame waits for the previous one)", 0)):
+        benchlib.frame_loop(bufs, cfg.M, out.SK, out.mask, ws, 50, flags, sk_mean=sk_mean, stream=stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        benchlib.frame_loop(bufs, cfg.M, out.SK, out.mask, ws, 200, flags, sk_mean=sk_mean, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        est = e0.elapsed_time(e1) * 1e-3 / 200
+        calls = max(200, int(args.seconds / est))
+        benchlib.frame_loop(bufs, cfg.M, out.SK, out.mask, ws, calls // 2, flags, sk_mean=sk_mean, stream=stream)
+        sampler = ClockSampler(0)
+        sampler.start()
+        torch.cuda.synchronize()
+        t_lo = time.perf_counter()
+        sampler.window = (t_lo, None)
+        e0.record(stream)
+        host_s = benchlib.frame_loop(bufs, cfg.M, out.SK, out.mask, ws, calls, flags, sk_mean=sk_mean, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        sampler.window = (t_lo, time.perf_counter())
+        clocks = sampler.summary()
+        sampler.stop_flag = True
+        per = e0.elapsed_time(e1) * 1e-3 / calls
+        # the host cost of a call by itself: 16 calls into an idle stream (the loop above runs at the device's
+        # pace once the launch queue is full, so its host time per call is just the device time again)
+        idle = []
+        for _ in range(20):
+            torch.cuda.synchronize()
+            idle.append(benchlib.frame_loop(bufs, cfg.M, out.SK, out.mask, ws, 16, flags, sk_mean=sk_mean, stream=stream) / 16)
+        torch.cuda.synchronize()
+        rows.append({"flags": name, "calls": calls, "us_per_frame": per * 1e6, "host_us_per_call": host_s / calls * 1e6,
+                     "host_us_per_call_idle_stream": sorted(idle)[len(idle) // 2] * 1e6,
+                     "samples_per_s": cfg.nbytes / per, "read_gbs": cfg.nbytes / per / 1e9,
+                     "frac_of_peak": cfg.nbytes / per / 1e9 / peak, "clocks": clocks})
+    print(json.dumps({
+        "op": "eager", "metric": METRIC, "value": rows[0]["samples_per_s"], "unit": UNIT, "n_gpus": 1,
+        "steps": rows[0]["calls"], "warmup": rows[0]["calls"] // 2, "ms_per_step": rows[0]["us_per_frame"] * 1e-3,
+        "higher_is_better": True, "data": "synthetic", "dtype": "u8->u32/f64",
+        "config": {"workload": cfg.name, "frame_bytes": cfg.nbytes, "frames": nbuf,
+                   "launch": "NO CUDA graph: plain back-to-back sk_frame calls from a C loop (skb_frame_loop), one stream",
+                   "peak_gbs": peak, "peak_source": peak_src},
+        "cases": rows, "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
 def frame_ids(rank, nbuf):
@@ -605,7 +751,7 @@ def run_sweep(args, sk, sk_synth, torch, dev):
             ms, reps, _ = timed_replays(torch, graph, stream, args.sweep_seconds, ms * 1e-3 / (reps * K), K,
                                         torch.cuda.synchronize)
             step_s = ms * 1e-3 / (reps * K)
-            lanes, slabs, chunk, bpu = sk.sk_debug_get_plan(cfg.T, cfg.F, cfg.E, M, first_n=N, inputs_ready=True)
+            lanes, slabs, chunk, bpu = sk.sk_frame_plan(cfg.T, cfg.F, cfg.E, M, first_n=N, inputs_ready=True)
             alg = cfg.T * cfg.F * N + B * cfg.F * 5                                  # N/E of the frame + outputs
             moved = cfg.T * cfg.F * min(cfg.E, slabs * 16 * lanes) + B * cfg.F * 5   # whole slabs are fetched
             skv = out.SK.double()
@@ -707,6 +853,10 @@ def main():
         return run_fig6(args)
     if args.op == "firstpass":
         return run_firstpass(args)
+    if args.op == "memonly":
+        return run_memonly(args)
+    if args.op == "eager":
+        return run_eager(args)
     if args.op != "frame":
         return run_aux(args)
 
@@ -727,7 +877,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     sk.lib()
     if args.path == "ldg" or args.lanes:
-        sk.sk_debug_set_plan(sk.SK_PLAN_LDG if args.path == "ldg" else sk.SK_PLAN_AUTO, args.lanes)
+        sk.plan_override(sk.SK_PLAN_LDG if args.path == "ldg" else sk.SK_PLAN_AUTO, args.lanes)
     if args.sweep:
         if world > 1:
             raise SystemExit("--sweep is a single-GPU line")

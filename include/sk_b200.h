@@ -21,8 +21,8 @@
  *     (a cudaStream_t cast to void*; NULL = the legacy default stream) before returning.
  *   - Return value: 0 = enqueued; < 0 = argument error (SK_ERR_*), nothing was enqueued;
  *     > 0 = a cudaError_t reported by a launch or copy.  No exceptions.  The only process-wide
- *     state is the launch counter (sk_launch_count), per-device caches of device attributes, and
- *     the test-only override of sk_debug_set_plan.
+ *     state is the launch counter (sk_launch_count) and per-device caches of device attributes and
+ *     of the address of sk_frame_noalloc's scratch; nothing a caller can set outlives its call.
  *   - Receiver selection ("total number of receivers"): `subset` is NULL or E
  *     bytes on the device (non-zero = combine this input).  With subset == NULL the first
  *     `first_n` inputs are combined (first_n = E for the whole array).  N is the number of
@@ -83,6 +83,14 @@ size_t sk_frame_workspace_bytes(uint32_t T, uint32_t F, uint32_t E, uint32_t M);
 #define SK_FRAME_EQ13          4  /* SK = the un-rescaled estimator of PAPER.md:97-104 Eq. 13,
                                    * (MN+1)/(MN-1) * (S2bar/(MN) - 1), instead of Eq. 14; the flag
                                    * interval is applied to it unchanged (pass the matching sk_mean) */
+/* Tests and A/B timing: override the library's kernel choice for THIS call (sk_frame, sk_frame_multi,
+ * sk_frame_noalloc, sk_frame_host, sk_frame_plan).  Results do not depend on any of them
+ * (DESIGN.md section 5.1): every kernel and slab width gives the same bits. */
+#define SK_FRAME_PLAN_LDG      (1 << 8)   /* the direct-load kernel instead of the TMA stream kernel */
+#define SK_FRAME_PLAN_NO_TMAP  (1 << 9)   /* plan as usual, then behave as if the driver had refused to encode
+                                           * the tensor map: exercises the fall-back to the direct-load kernels */
+#define SK_FRAME_PLAN_LANES(l) (((l) & 31) << 12)   /* l = 1, 2, 4, 8, 16: slab width 16*l inputs, if not wider
+                                                     * than a row; 0 = automatic */
 
 /* a1-a8 in one pass over HBM.  Writes SK and mask [T/M][F]; S1_opt / S2_opt [T/M][F][E] are
  * written when non-NULL.  With SK_FRAME_ZERO_FLAGGED every byte (all E inputs, all M rows) of
@@ -228,42 +236,14 @@ int sk_version(void);
  * gpu_launches count; monotonically increasing, thread-safe). */
 unsigned long long sk_launch_count(void);
 
-/* Tests and A/B timing only: override the kernel choice of the fused path for the whole process.
- * path = SK_PLAN_AUTO (default), SK_PLAN_LDG (direct-load kernel instead of the TMA stream
- * kernel) or SK_PLAN_NO_TMAP; lanes = 0 (automatic) or 1, 2, 4, 8, 16: slab width 16*lanes inputs, if not wider than
- * a row.  Results do not depend on either. */
-#define SK_PLAN_AUTO 0
-#define SK_PLAN_LDG  1
-#define SK_PLAN_NO_TMAP 2   /* plan as usual, but behave as if the driver had refused to encode the tensor
-                             * map: exercises the fall-back to the direct-load kernels (identical results) */
-void sk_debug_set_plan(int path, int lanes);
-
-/* Tests and bench reporting only: the launch plan sk_frame / sk_frame_multi would use for this
- * shape with a 16-byte-aligned `data` and no subset.  plan4 (HOST, 4 words) = { lanes (slab width
- * / 16), slabs launched per cell (only those covering first_n), rows per accumulator read-out of
- * the TMA stream kernel or 0 when the direct-load kernel would run, M-row blocks per unit }. */
-int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags,
-                      uint32_t nlev, uint32_t* plan4);
-
-/* Measurement only (bench.py --op ceiling): the SM-side ceiling of the hot loop.
- * Runs the stream kernel's tile loop (a1-a3 on 128-bit shared-memory reads) on a fixed shared-memory
- * tile with no global-memory traffic: one CTA per SM, warps_per_sm (1..16) warps each, `rounds` x 8
- * tiles of 8 KiB per warp.  sink: device, (SM count) * warps_per_sm * 32 words, written (keeps the
- * arithmetic alive); cycles: device, one 64-bit word = elapsed SM clocks of CTA 0;
- * h_samples_per_lane (HOST, may be NULL) = samples every lane has added.  Sub-partition cycles per
- * 32 samples = cycles / (samples_per_lane * warps_per_sm / 4), warps_per_sm a multiple of 4. */
-int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink, unsigned long long* cycles,
-                          double* h_samples_per_lane, void* stream);
-
-/* Measurement only (bench.py --op ceiling): issue rate of the hot loop's instructions, alone and in
- * pairs, 8 independent chains per lane.  mode: 0 FFMA, 1 FFMA2 (fma.rn.f32x2), 2 FADD2 (sub.rn.f32x2),
- * 3 IDP.4A (dp4a), 4 PRMT, 5 IDP + FFMA2, 6 IDP + FFMA, 7 PRMT + FFMA2, 8 IDP + PRMT.  io: device,
- * 2048 + (SM count) * warps_per_sm * 32 words (the first 2048 are read as operands, the rest written);
- * cycles: device, elapsed SM clocks of CTA 0; h_instructions_per_warp (HOST, may be NULL) = warp
- * instructions every warp issued.  Sub-partition cycles per instruction = cycles / (instructions *
- * warps_per_sm / 4). */
-int sk_debug_pipe_rate(int mode, uint32_t warps_per_sm, uint32_t* io, unsigned long long* cycles,
-                       double* h_instructions_per_warp, void* stream);
+/* The launch plan sk_frame / sk_frame_multi would use for this shape with a 16-byte-aligned `data`
+ * and no subset (a pure function of its arguments and the device's SM count; for tests and for
+ * bench reporting).  flags: SK_FRAME_INPUTS_READY and the SK_FRAME_PLAN_* bits matter.  plan4 (HOST,
+ * 4 words) = { lanes (slab width / 16), slabs launched per cell (only those covering first_n), rows
+ * per accumulator read-out of the TMA stream kernel or 0 when the direct-load kernel would run,
+ * M-row blocks per unit }. */
+int sk_frame_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags,
+                  uint32_t nlev, uint32_t* plan4);
 
 #ifdef __cplusplus
 }

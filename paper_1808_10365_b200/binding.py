@@ -17,11 +17,12 @@ SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes",
            "sk_frame_noalloc",
            "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
            "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
-           "sk_launch_count", "sk_debug_set_plan", "sk_debug_get_plan", "sk_debug_loop_ceiling", "sk_debug_pipe_rate")
+           "sk_launch_count", "sk_frame_plan")
 
 # bits of sk_frame's `flags` (include/sk_b200.h)
 SK_FRAME_ZERO_FLAGGED, SK_FRAME_INPUTS_READY, SK_FRAME_EQ13 = 1, 2, 4
-SK_PLAN_AUTO, SK_PLAN_LDG, SK_PLAN_NO_TMAP = 0, 1, 2
+SK_FRAME_PLAN_LDG, SK_FRAME_PLAN_NO_TMAP = 1 << 8, 1 << 9
+SK_PLAN_AUTO, SK_PLAN_LDG, SK_PLAN_NO_TMAP = 0, 1, 2      # arguments of plan_override (Python side only)
 
 _lib = None
 
@@ -57,14 +58,8 @@ def lib() -> C.CDLL:
     L.sk_frame_multi_workspace_bytes.argtypes = [u32, u32, u32, u32, u32]
     L.sk_frame_multi_workspace_bytes.restype = sz
     L.sk_frame_multi.argtypes = [vp, u32, u32, u32, u32, u32, vp, u32, f32, vp, i32, vp, vp, vp, sz, vp]
-    L.sk_debug_set_plan.argtypes = [i32, i32]
-    L.sk_debug_set_plan.restype = None
-    L.sk_debug_get_plan.argtypes = [u32, u32, u32, u32, u32, i32, u32, vp]
-    L.sk_debug_get_plan.restype = i32
-    L.sk_debug_loop_ceiling.argtypes = [u32, u32, vp, vp, vp, vp]
-    L.sk_debug_loop_ceiling.restype = i32
-    L.sk_debug_pipe_rate.argtypes = [i32, u32, vp, vp, vp, vp]
-    L.sk_debug_pipe_rate.restype = i32
+    L.sk_frame_plan.argtypes = [u32, u32, u32, u32, u32, i32, u32, vp]
+    L.sk_frame_plan.restype = i32
     L.sk_rebin_sums.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     L.sk_single.argtypes = [vp, vp, u32, u32, u32, u32, vp, vp]
     L.sk_significance.argtypes = [vp, u32, u32, u32, u32, f32, vp, vp]
@@ -94,53 +89,34 @@ def sk_launch_count() -> int:
     return int(lib().sk_launch_count())
 
 
-def sk_debug_set_plan(path: int = SK_PLAN_AUTO, lanes: int = 0) -> None:
-    """Tests and A/B timing only (include/sk_b200.h): force the direct-load kernel and / or a
-    narrower slab width for the whole process.  (0, 0) restores the automatic choice."""
-    lib().sk_debug_set_plan(int(path), int(lanes))
+_plan_flags = 0      # SK_FRAME_PLAN_* bits added to the flags of every fused call made through this module
 
 
-def sk_debug_get_plan(T: int, F: int, E: int, M: int, first_n=None, inputs_ready: bool = False, nlev: int = 1):
+def plan_flags(path: int = SK_PLAN_AUTO, lanes: int = 0) -> int:
+    """The SK_FRAME_PLAN_* bits of include/sk_b200.h for a kernel path and a slab width of 16*lanes inputs."""
+    f = SK_FRAME_PLAN_LDG if path == SK_PLAN_LDG else SK_FRAME_PLAN_NO_TMAP if path == SK_PLAN_NO_TMAP else 0
+    if lanes in (1, 2, 4, 8, 16):
+        f |= lanes << 12
+    return f
+
+
+def plan_override(path: int = SK_PLAN_AUTO, lanes: int = 0) -> None:
+    """Tests and A/B timing only: from now on every sk_frame / sk_frame_multi / sk_frame_host /
+    sk_frame_noalloc call made through THIS module passes the SK_FRAME_PLAN_* bits for `path` and `lanes`
+    (the direct-load kernel, a refused tensor map, a narrower slab) in its flags.  The C library itself keeps
+    no such state: the override is per call.  (0, 0) restores the automatic choice."""
+    global _plan_flags
+    _plan_flags = plan_flags(path, lanes)
+
+
+def sk_frame_plan(T: int, F: int, E: int, M: int, first_n=None, inputs_ready: bool = False, nlev: int = 1,
+                  flags=None):
     """(lanes, slabs, chunk_rows or 0 for the direct-load kernel, blocks_per_unit) the fused path
-    would use for this shape (aligned data, no subset).  Tests and bench reporting only."""
+    would use for this shape (aligned data, no subset) under the current plan_override (or `flags`)."""
     plan = (C.c_uint32 * 4)()
-    _check(lib().sk_debug_get_plan(T, F, E, M, int(first_n or E), SK_FRAME_INPUTS_READY if inputs_ready else 0,
-                                   nlev, C.cast(plan, C.c_void_p)), "sk_debug_get_plan")
+    fl = (_plan_flags if flags is None else int(flags)) | (SK_FRAME_INPUTS_READY if inputs_ready else 0)
+    _check(lib().sk_frame_plan(T, F, E, M, int(first_n or E), fl, nlev, C.cast(plan, C.c_void_p)), "sk_frame_plan")
     return tuple(int(x) for x in plan)
-
-
-def sk_debug_loop_ceiling(warps_per_sm: int = 12, rounds: int = 200, device="cuda") -> float:
-    """Measurement only (include/sk_b200.h): sub-partition cycles per 32 samples of the hot loop on a
-    fixed shared-memory tile, no global-memory traffic.  Synchronises."""
-    dev = torch.device(device)
-    if dev.type != "cuda":
-        raise SKError("sk_debug_loop_ceiling needs a CUDA device")
-    sms = torch.cuda.get_device_properties(dev).multi_processor_count
-    sink = torch.empty(sms * warps_per_sm * 32, dtype=torch.int32, device=dev)
-    cycles = torch.zeros(1, dtype=torch.int64, device=dev)
-    spl = C.c_double(0.0)
-    _check(lib().sk_debug_loop_ceiling(warps_per_sm, rounds, sink.data_ptr(), cycles.data_ptr(),
-                                       C.cast(C.pointer(spl), C.c_void_p), _cur()), "sk_debug_loop_ceiling")
-    torch.cuda.synchronize(dev)
-    return float(cycles.item()) / (spl.value * warps_per_sm / 4.0)
-
-
-PIPE_MODES = ("FFMA", "FFMA2", "FADD2", "IDP.4A", "PRMT", "IDP+FFMA2", "IDP+FFMA", "PRMT+FFMA2", "IDP+PRMT")
-
-
-def sk_debug_pipe_rate(mode: int, warps_per_sm: int = 16, device="cuda") -> float:
-    """Measurement only (include/sk_b200.h): sub-partition cycles per warp instruction of PIPE_MODES[mode]."""
-    dev = torch.device(device)
-    if dev.type != "cuda":
-        raise SKError("sk_debug_pipe_rate needs a CUDA device")
-    sms = torch.cuda.get_device_properties(dev).multi_processor_count
-    io = torch.full((2048 + sms * warps_per_sm * 32,), 0x3F800011, dtype=torch.int32, device=dev)
-    cycles = torch.zeros(1, dtype=torch.int64, device=dev)
-    n = C.c_double(0.0)
-    _check(lib().sk_debug_pipe_rate(mode, warps_per_sm, io.data_ptr(), cycles.data_ptr(),
-                                    C.cast(C.pointer(n), C.c_void_p), _cur()), "sk_debug_pipe_rate")
-    torch.cuda.synchronize(dev)
-    return float(cycles.item()) / (n.value * warps_per_sm / 4.0)
 
 
 def _check(rc: int, what: str):
@@ -364,7 +340,7 @@ def sk_frame(data: torch.Tensor, M: int, subset=None, first_n=None, n_sigma: flo
         if workspace is None:
             workspace = workspace_for(T, F, E, M, dev, ts.cuda_stream)
         flags = ((SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_INPUTS_READY if inputs_ready else 0)
-                 | (SK_FRAME_EQ13 if eq13 else 0))
+                 | (SK_FRAME_EQ13 if eq13 else 0) | _plan_flags)
         _check(lib().sk_frame(data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
                               flags, out.SK.data_ptr(), out.mask.data_ptr(), _ptr(out.S1), _ptr(out.S2),
                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
@@ -407,7 +383,7 @@ def sk_frame_noalloc(data: torch.Tensor, M: int, out: SKResult, subset: Optional
     elif first_n is None:
         first_n = E
     ts = _torch_stream(stream, data.device)
-    flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_EQ13 if eq13 else 0)
+    flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_EQ13 if eq13 else 0) | _plan_flags
     with torch.cuda.device(data.device):        # the scratch's address is looked up on the current device
         _check(lib().sk_frame_noalloc(data.data_ptr(), T, F, E, M, _ptr(subset), int(first_n or 0), n_sigma, sk_mean,
                                       flags, out.SK.data_ptr(), out.mask.data_ptr(), _ptr(out.S1), _ptr(out.S2),
@@ -449,7 +425,7 @@ def sk_frame_multi(data: torch.Tensor, M: int, nlev: int, subset=None, first_n=N
         c_means = (C.c_float * nlev)(*means)
         c_SK = (C.c_void_p * nlev)(*[t.data_ptr() for t in out.SK])
         c_mask = (C.c_void_p * nlev)(*[t.data_ptr() for t in out.mask])
-        flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_INPUTS_READY if inputs_ready else 0)
+        flags = (SK_FRAME_ZERO_FLAGGED if zero_flagged else 0) | (SK_FRAME_INPUTS_READY if inputs_ready else 0) | _plan_flags
         _check(lib().sk_frame_multi(data.data_ptr(), T, F, E, M, nlev, _ptr(sub), int(first_n or 0), n_sigma,
                                     C.cast(c_means, C.c_void_p), flags, C.cast(c_SK, C.c_void_p),
                                     C.cast(c_mask, C.c_void_p), workspace.data_ptr(),
@@ -474,7 +450,7 @@ def sk_frame_host(h_data: torch.Tensor, M: int, h_SK: torch.Tensor, h_mask: torc
         if workspace is None:
             workspace = workspace_for(T, F, E, M, d_data.device, ts.cuda_stream)
         _check(lib().sk_frame_host(h_data.data_ptr(), T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma,
-                                   sk_mean, int(bool(zero_flagged)), h_SK.data_ptr(), h_mask.data_ptr(),
+                                   sk_mean, int(bool(zero_flagged)) | _plan_flags, h_SK.data_ptr(), h_mask.data_ptr(),
                                    d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
                                    workspace.numel() * workspace.element_size(), ts.cuda_stream), "sk_frame_host")
     return h_SK, h_mask

@@ -7,15 +7,19 @@
 // 8 tiles (128 samples per lane: AccChain2's limit) as in the kernel.  The elapsed SM cycles of
 // CTA 0 give the cycles one sub-partition needs per 32 samples (one sample per lane) — what the
 // instruction mix costs when nothing else is in the way.  bench.py reports it beside the roofline
-// (DESIGN.md section 6); no product path calls this.
+// (DESIGN.md section 6).  VAR = kVarProduct is the product's loop body; kVarNoSub / kVarNoPick /
+// kVarNoUnpack leave one kind of instruction out (sk_device.cuh), which is how DESIGN.md section 6.3
+// attributes the loop's cycles to pipes.  Part of the bench library only (libsk_b200_bench.so): the
+// product library contains none of this.
 #pragma once
-#include "sk_tma.cuh"
+#include "../sk_tma.cuh"
 
 namespace sk {
 
 constexpr int kCeilingMaxWarps = 16;
 constexpr int kCeilingTilesPerReadout = 8;
 
+template <int VAR>
 __global__ void __launch_bounds__(kCeilingMaxWarps * 32)
 sk_loop_ceiling_kernel(uint32_t* __restrict__ sink, unsigned long long* __restrict__ cycles, uint32_t rounds) {
     constexpr int L = 16, RPW = 32 / L, W = 16 * L, NLD = kTileBytes / W / RPW;
@@ -35,7 +39,7 @@ sk_loop_ceiling_kernel(uint32_t* __restrict__ sink, unsigned long long* __restri
         for (int k = 0; k < 8; ++k) acc[k].reset();
         for (int g = 0; g < kCeilingTilesPerReadout; ++g) {
 #pragma unroll
-            for (int i = 0; i < NLD; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+            for (int i = 0; i < NLD; ++i) accumulate16<AccChain2, VAR>(acc, lds128(src + i * RPW * W), kc);
             __syncwarp();
         }
         uint32_t S1[16], S2[16];

@@ -9,14 +9,27 @@
 #include "sk_kernels.cuh"
 #include "sk_tma.cuh"
 #include "sk_sim.cuh"
-#include "sk_ceiling.cuh"
 
 namespace {
 
-std::atomic<unsigned long long> g_launches{0};
-// sk_debug_set_plan (tests and A/B timing only): 0 = automatic
-std::atomic<int> g_force_path{0};     // SK_PLAN_LDG: never the stream kernel
-std::atomic<int> g_force_lanes{0};    // a (narrower) slab width of 16 * lanes inputs
+std::atomic<unsigned long long> g_launches{0};      // the library's only mutable process-wide state
+
+// The SK_FRAME_PLAN_* bits of a call's `flags` (tests and A/B timing): they override the kernel
+// choice for that call only.  Default-constructed = automatic.
+struct Force {
+    bool ldg = false;        // never the stream kernel
+    bool no_tmap = false;    // behave as if the driver had refused to encode the tensor map
+    int lanes = 0;           // != 0: a slab width of 16 * lanes inputs
+};
+
+Force force_of(int flags) {
+    Force fc;
+    fc.ldg = (flags & SK_FRAME_PLAN_LDG) != 0;
+    fc.no_tmap = (flags & SK_FRAME_PLAN_NO_TMAP) != 0;
+    const int l = (flags >> 12) & 31;
+    if (l >= 1 && l <= 16 && (l & (l - 1)) == 0) fc.lanes = l;
+    return fc;
+}
 
 inline int launch_status() {
     const cudaError_t e = cudaGetLastError();
@@ -49,13 +62,13 @@ int sm_count() {
 // SM enough warps; otherwise narrower slabs.  A lone frame needs ~16 warps per SM of its own;
 // frames that overlap their neighbours on the stream (SK_FRAME_INPUTS_READY) share the SM with
 // them and run best on wide slabs from 8 warps per SM up (measured on config 1: 16.3 vs 17.0 us).
-inline int lanes_per_row(uint32_t E, unsigned long long units_per_slab_column, bool overlapped) {
+inline int lanes_per_row(uint32_t E, unsigned long long units_per_slab_column, bool overlapped, const Force& fc) {
     const uint32_t vecs = E / 16;            // 128-bit vectors per row
     int L = 16;
     while (L > 1 && (uint32_t)L > vecs) L >>= 1;
     const unsigned long long want = (unsigned long long)sm_count() * (overlapped ? 8u : 16u);
     while (L > 4 && units_per_slab_column * ((E + 16u * L - 1) / (16u * L)) < want) L >>= 1;
-    const int v = g_force_lanes.load(std::memory_order_relaxed);
+    const int v = fc.lanes;
     if (v >= 1 && (uint32_t)v <= (vecs < 16u ? vecs : 16u) && (v & (v - 1)) == 0) L = v;
     return L;
 }
@@ -99,7 +112,7 @@ struct Plan {
 
 // nlev = integration lengths wanted (M << 0 .. M << (nlev-1)); B % (1 << (nlev-1)) == 0.
 Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F, const uint8_t* subset,
-               uint32_t first_n, bool need_all_inputs, bool overlapped, uint32_t nlev) {
+               uint32_t first_n, bool need_all_inputs, bool overlapped, uint32_t nlev, const Force& fc = Force{}) {
     Plan pl{};
     pl.vec = vector_ok(data, E);
     // blocks per unit: the longest length's worth, and for short blocks as many as make a unit
@@ -110,11 +123,11 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
            (unsigned long long)(B / (2u * bpu)) * F * ((E + 255u) / 256u) >= want)
         bpu *= 2u;
     pl.bpu = bpu;
-    pl.L = lanes_per_row(E, (unsigned long long)(B / bpu) * F, overlapped);
+    pl.L = lanes_per_row(E, (unsigned long long)(B / bpu) * F, overlapped, fc);
     uint32_t cover = E;
     if (!subset && !need_all_inputs) cover = first_n;    // inputs beyond first_n are never read
     // a few receivers only: one slab no wider than needed (64 bytes at least), so that the rest of the row is not fetched
-    while (pl.L > 4 && 8u * pl.L >= cover && g_force_lanes.load(std::memory_order_relaxed) == 0) pl.L >>= 1;
+    while (pl.L > 4 && 8u * pl.L >= cover && fc.lanes == 0) pl.L >>= 1;
     const uint32_t W = 16u * pl.L;
     pl.slabs = (cover + W - 1) / W;
     const uint32_t RPW = 32u / pl.L;
@@ -129,7 +142,7 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     const bool grid_ok = B / bpu <= 65535u && F <= 65535u && (unsigned long long)F * E + 256ull <= (1ull << 31) &&
                          (unsigned long long)B * M < (1ull << 31);
     pl.chunk = (pl.vec && grid_ok && pl.L >= 4) ? chunk_rows(M, pl.L) : 0u;
-    if (pl.chunk == 0u && pl.vec && grid_ok && g_force_lanes.load(std::memory_order_relaxed) == 0) {
+    if (pl.chunk == 0u && pl.vec && grid_ok && fc.lanes == 0) {
         // the block length is not a whole number of tiles at this slab width (a tile is 8 KiB: 32 rows of
         // 256 B, 64 of 128 B, 128 of 64 B): a wider slab has shorter tiles; take the first width that fits
         int widest = 16;                                  // ... but no wider than the receivers asked for justify
@@ -148,9 +161,9 @@ Plan make_plan(const void* data, uint32_t E, uint32_t M, uint32_t B, uint32_t F,
     if (pl.chunk == 0u && pl.vec && grid_ok && nlev == 1) {
         // no slab width makes the block a whole number of tiles: the ragged stream kernel, at the widest
         // slab (shortest tiles), as long as the block is at least two tiles long
-        int L2 = g_force_lanes.load(std::memory_order_relaxed) ? pl.L : 16;
+        int L2 = fc.lanes ? pl.L : 16;
         while (L2 > 1 && (uint32_t)L2 > E / 16) L2 >>= 1;
-        while (L2 > 4 && 8u * L2 >= cover && g_force_lanes.load(std::memory_order_relaxed) == 0) L2 >>= 1;
+        while (L2 > 4 && 8u * L2 >= cover && fc.lanes == 0) L2 >>= 1;
         const uint32_t R = sk::kTileBytes / (16u * (uint32_t)L2);
         const uint32_t it2 = (M + 32u / L2 - 1) / (32u / L2);            // samples a lane adds per block
         // worth it for long blocks only: up to 128 samples per lane the direct-load kernel keeps the packed
@@ -206,9 +219,9 @@ EncodeTiledFn encode_tiled() {
     return fn;
 }
 
-// The stream kernel runs whenever it applies; sk_debug_set_plan(SK_PLAN_LDG, ..) turns it off.
-bool stream_wanted(const Plan& pl) {
-    if (g_force_path.load(std::memory_order_relaxed) == SK_PLAN_LDG) return false;
+// The stream kernel runs whenever it applies; SK_FRAME_PLAN_LDG turns it off for the call.
+bool stream_wanted(const Plan& pl, const Force& fc) {
+    if (fc.ldg) return false;
     return (pl.chunk != 0 || pl.ragged_tpb != 0) && encode_tiled() != nullptr;
 }
 
@@ -279,7 +292,7 @@ int launch_stream_L(const CUtensorMap& tmap, const sk::FrameParams& p, bool chun
 // callers fall back to the direct-load kernels, whose results are identical.  Never returned to a user.
 constexpr int kEncodeFailed = -1000;
 
-int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
+int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st, const Force& fc) {
     CUtensorMap tmap;
     const uint32_t W = 16u * pl.L;
     const cuuint64_t gdim[2] = {(cuuint64_t)p.F * p.E, (cuuint64_t)p.T};
@@ -289,7 +302,7 @@ int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     const CUresult r = encode_tiled()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(p.data), gdim,
                                       gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS || g_force_path.load(std::memory_order_relaxed) == SK_PLAN_NO_TMAP) return kEncodeFailed;
+    if (r != CUDA_SUCCESS || fc.no_tmap) return kEncodeFailed;
     const bool chunked = pl.chunk != p.M;
     const uint32_t zblocks = p.B / pl.bpu;
     int rc;
@@ -311,18 +324,18 @@ int launch_stream(const Plan& pl, const sk::FrameParams& p, cudaStream_t st) {
     return rc;
 }
 
-int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st) {
+int launch_cells(const Plan& pl, sk::FrameParams& p, cudaStream_t st, const Force& fc = Force{}) {
     const uint32_t cells = p.B * p.F;
     if (pl.vec) {
         p.slabs = pl.slabs;
         p.nunits = cells * pl.slabs;
         int rc = kEncodeFailed;                                    // "no stream kernel": also when it is not wanted
-        if (stream_wanted(pl)) {
+        if (stream_wanted(pl, fc)) {
             p.chunk = pl.chunk;
             p.bpu = pl.bpu;
             p.tpb = pl.ragged_tpb;
             p.unit_tiles = pl.ragged_tpb ? pl.ragged_tpb * pl.bpu : p.M * pl.bpu / (sk::kTileBytes / (16u * pl.L));
-            rc = launch_stream(pl, p, st);
+            rc = launch_stream(pl, p, st, fc);
             if (rc != SK_OK && rc != kEncodeFailed) return rc;
             if (rc == kEncodeFailed && p.nlev > 1) return rc;      // frame_impl takes one pass per length instead
         }
@@ -383,7 +396,8 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
     if ((flags & SK_FRAME_ZERO_FLAGGED) && !mask[0]) return SK_ERR_NULL;
     if (int rc = check_frame_args(subset, E, first_n, n_sigma, sk_means, nlev, any_mask)) return rc;
     if ((S1o == nullptr) != (S2o == nullptr)) return SK_ERR_NULL;
-    Plan pl = make_plan(data, E, M, B, F, subset, first_n, S1o != nullptr, (flags & SK_FRAME_INPUTS_READY) != 0, nlev);
+    const Force fc = force_of(flags);
+    Plan pl = make_plan(data, E, M, B, F, subset, first_n, S1o != nullptr, (flags & SK_FRAME_INPUTS_READY) != 0, nlev, fc);
     if (S1o && ((reinterpret_cast<uintptr_t>(S1o) | reinterpret_cast<uintptr_t>(S2o)) & 15u)) pl.vec = false;
     sk::FrameParams p{};
     p.data = data; p.T = T; p.F = F; p.E = E; p.M = M; p.B = B;
@@ -394,7 +408,7 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
     p.eq13 = (flags & SK_FRAME_EQ13) ? 1u : 0u;
     p.inputs_ready = (flags & SK_FRAME_INPUTS_READY) ? 1u : 0u;
     p.S1out = S1o; p.S2out = S2o;
-    const bool one_launch = nlev == 1 || (pl.vec && stream_wanted(pl));
+    const bool one_launch = nlev == 1 || (pl.vec && stream_wanted(pl, fc));
     if (pl.vec) {
         if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) ||
             workspace_bytes_given < workspace_bytes(B, F, E, nlev))
@@ -414,7 +428,7 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
         }
     }
     if (one_launch) {
-        const int rc = launch_cells(pl, p, st);
+        const int rc = launch_cells(pl, p, st, fc);
         if (rc != kEncodeFailed) return rc;                        // only with nlev > 1: no tensor map, take the passes below
     }
     // several lengths without the stream kernel: one pass of the fused path per length, then the
@@ -425,9 +439,9 @@ int frame_impl(const uint8_t* data, uint32_t T, uint32_t F, uint32_t E, uint32_t
         pl_l.lev[0] = p.lev[l];
         pl_l.S1out = l == 0 ? S1o : nullptr; pl_l.S2out = l == 0 ? S2o : nullptr;
         pl_l.inputs_ready = l == 0 ? p.inputs_ready : 0u;
-        Plan q = make_plan(data, E, M << l, B >> l, F, subset, first_n, pl_l.S1out != nullptr, false, 1);
+        Plan q = make_plan(data, E, M << l, B >> l, F, subset, first_n, pl_l.S1out != nullptr, false, 1, fc);
         q.vec = pl.vec;
-        if (int rc = launch_cells(q, pl_l, st)) return rc;
+        if (int rc = launch_cells(q, pl_l, st, fc)) return rc;
     }
     for (uint32_t l = 0; l < nlev && p.excise; ++l) {
         if (!mask[l]) continue;
@@ -612,7 +626,7 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
     const size_t bytes = (size_t)T * F * E, cells = (size_t)(T / M) * F;
     cudaError_t e = cudaMemcpyAsync(d_data, h_data, bytes, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return (int)e;
-    const int keep = flags & (SK_FRAME_ZERO_FLAGGED | SK_FRAME_EQ13);
+    const int keep = flags & ~SK_FRAME_INPUTS_READY;
     int rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, keep, d_SK, d_mask, nullptr,
                       nullptr, workspace, workspace_bytes_given, stream);
     if (rc == SK_OK) {
@@ -735,60 +749,20 @@ int sk_version(void) { return 200; }
 
 unsigned long long sk_launch_count(void) { return g_launches.load(); }
 
-int sk_debug_get_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags, uint32_t nlev,
-                      uint32_t* plan4) {
+int sk_frame_plan(uint32_t T, uint32_t F, uint32_t E, uint32_t M, uint32_t first_n, int flags, uint32_t nlev,
+                  uint32_t* plan4) {
     if (!plan4) return SK_ERR_NULL;
     if (int rc = check_shape(T, F, E, M)) return rc;
     if (nlev < 1 || nlev > (uint32_t)sk::kMaxLevels || (T / M) % (1u << (nlev - 1)) != 0) return SK_ERR_SHAPE;
     if (first_n == 0 || first_n > E) return SK_ERR_N;
     // an aligned data pointer is assumed (the vector path)
-    const Plan pl = make_plan(nullptr, E, M, T / M, F, nullptr, first_n, false, (flags & SK_FRAME_INPUTS_READY) != 0, nlev);
+    const Force fc = force_of(flags);
+    const Plan pl = make_plan(nullptr, E, M, T / M, F, nullptr, first_n, false, (flags & SK_FRAME_INPUTS_READY) != 0, nlev, fc);
     plan4[0] = (uint32_t)pl.L;
     plan4[1] = pl.slabs;
-    plan4[2] = (pl.vec && stream_wanted(pl)) ? (pl.ragged_tpb ? sk::kRaggedTilesPerReadout * sk::kTileBytes / (16u * pl.L) : pl.chunk) : 0u;
+    plan4[2] = (pl.vec && stream_wanted(pl, fc)) ? (pl.ragged_tpb ? sk::kRaggedTilesPerReadout * sk::kTileBytes / (16u * pl.L) : pl.chunk) : 0u;
     plan4[3] = pl.bpu;
     return SK_OK;
-}
-
-int sk_debug_loop_ceiling(uint32_t warps_per_sm, uint32_t rounds, uint32_t* sink, unsigned long long* cycles,
-                          double* h_samples_per_lane, void* stream) {
-    if (!sink || !cycles) return SK_ERR_NULL;
-    if (warps_per_sm < 1 || warps_per_sm > (uint32_t)sk::kCeilingMaxWarps || rounds == 0) return SK_ERR_SHAPE;
-    const size_t smem = (size_t)warps_per_sm * sk::kTileBytes;
-    cudaFuncSetAttribute(sk::sk_loop_ceiling_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    sk::sk_loop_ceiling_kernel<<<sm_count(), warps_per_sm * 32, smem, (cudaStream_t)stream>>>(sink, cycles, rounds);
-    ++g_launches;
-    // samples every lane of every warp has added: rounds x 8 tiles x 256 samples per lane and tile
-    if (h_samples_per_lane) *h_samples_per_lane = (double)rounds * sk::kCeilingTilesPerReadout * (sk::kTileBytes / 32);
-    return launch_status();
-}
-
-int sk_debug_pipe_rate(int mode, uint32_t warps_per_sm, uint32_t* io, unsigned long long* cycles,
-                       double* h_instructions_per_warp, void* stream) {
-    if (!io || !cycles) return SK_ERR_NULL;
-    if (mode < 0 || mode >= sk::kPipeModes || warps_per_sm < 1 || warps_per_sm > (uint32_t)sk::kCeilingMaxWarps)
-        return SK_ERR_SHAPE;
-    const unsigned grid = (unsigned)sm_count(), block = warps_per_sm * 32;
-    cudaStream_t st = (cudaStream_t)stream;
-    switch (mode) {
-        case 0: sk::sk_pipe_rate_kernel<0><<<grid, block, 0, st>>>(io, cycles); break;
-        case 1: sk::sk_pipe_rate_kernel<1><<<grid, block, 0, st>>>(io, cycles); break;
-        case 2: sk::sk_pipe_rate_kernel<2><<<grid, block, 0, st>>>(io, cycles); break;
-        case 3: sk::sk_pipe_rate_kernel<3><<<grid, block, 0, st>>>(io, cycles); break;
-        case 4: sk::sk_pipe_rate_kernel<4><<<grid, block, 0, st>>>(io, cycles); break;
-        case 5: sk::sk_pipe_rate_kernel<5><<<grid, block, 0, st>>>(io, cycles); break;
-        case 6: sk::sk_pipe_rate_kernel<6><<<grid, block, 0, st>>>(io, cycles); break;
-        case 7: sk::sk_pipe_rate_kernel<7><<<grid, block, 0, st>>>(io, cycles); break;
-        default: sk::sk_pipe_rate_kernel<8><<<grid, block, 0, st>>>(io, cycles); break;
-    }
-    ++g_launches;
-    if (h_instructions_per_warp) *h_instructions_per_warp = (double)sk::kPipeIters * 8 * (mode >= 5 ? 2 : 1);
-    return launch_status();
-}
-
-void sk_debug_set_plan(int path, int lanes) {
-    g_force_path.store((path == SK_PLAN_LDG || path == SK_PLAN_NO_TMAP) ? path : SK_PLAN_AUTO);
-    g_force_lanes.store((lanes >= 1 && lanes <= 16 && (lanes & (lanes - 1)) == 0) ? lanes : 0);
 }
 
 }  // extern "C"

@@ -139,11 +139,13 @@ struct AccChain2 {
     static constexpr uint32_t kMagic = 0x4B000000u;
     static constexpr uint32_t kMaxSamples = 128;
     __device__ __forceinline__ void reset() { r0 = r1 = kMagic; s2 = 0ull; }
+    // NOSUB (measurement builds only, see kVar* below): leave the FADD2 out; the sums are then wrong.
+    template <bool NOSUB = false>
     __device__ __forceinline__ void add2(uint32_t c0, uint32_t c1) {
         const uint32_t n0 = (uint32_t)__dp4a((int)c0, (int)c0, (int)r0);
         const uint32_t n1 = (uint32_t)__dp4a((int)c1, (int)c1, (int)r1);
-        unsigned long long d;
-        asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pack2(n0, n1)), "l"(pack2(r0, r1)));
+        unsigned long long d = pack2(n0, n1);
+        if (!NOSUB) asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pack2(n0, n1)), "l"(pack2(r0, r1)));
         asm("fma.rn.f32x2 %0, %1, %1, %2;" : "=l"(s2) : "l"(d), "l"(s2));
         r0 = n0;
         r1 = n1;
@@ -163,15 +165,41 @@ __device__ __forceinline__ uint32_t pick(uint32_t r16, uint32_t i16) {
     return __byte_perm(r16, i16, sel);
 }
 
+// Measurement variants of the loop body.  The product library instantiates
+// kVarProduct only; the others exist in the bench library (csrc/bench/), give WRONG sums by design and
+// answer one question each: what does the loop cost without this instruction?
+//   kVarMemOnly  : no arithmetic at all, the loaded words are XORed into the accumulators (is memory the limit?)
+//   kVarNoSub    : without the FADD2 (sub.rn.f32x2)          kVarNoPick : without the PRMTs (pick<K>)
+//   kVarNoUnpack : without the LOP3 / SHF / LOP3 of re16 / im16
+enum { kVarProduct = 0, kVarMemOnly = 1, kVarNoSub = 2, kVarNoPick = 3, kVarNoUnpack = 4 };
+
 // Add the 16 samples of one 128-bit load to the lane's 16 inputs (8 pair accumulators).
-template <class Acc2>
+template <class Acc2, int VAR = kVarProduct>
 __device__ __forceinline__ void accumulate16(Acc2 (&acc)[8], const uint4& v, const UnpackConsts& kc) {
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    if constexpr (VAR == kVarProduct) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
-        acc[2 * i + 0].add2(pick<0>(r, m), pick<1>(r, m));
-        acc[2 * i + 1].add2(pick<2>(r, m), pick<3>(r, m));
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t r = re16(w[i], kc), m = im16(w[i], kc);
+            acc[2 * i + 0].add2(pick<0>(r, m), pick<1>(r, m));
+            acc[2 * i + 1].add2(pick<2>(r, m), pick<3>(r, m));
+        }
+    } else if constexpr (VAR == kVarMemOnly) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[i].r0 ^= w[i];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t r = VAR == kVarNoUnpack ? w[i] : re16(w[i], kc);
+            const uint32_t m = VAR == kVarNoUnpack ? w[(i + 1) & 3] : im16(w[i], kc);
+            if constexpr (VAR == kVarNoPick) {
+                acc[2 * i + 0].add2(r, m);
+                acc[2 * i + 1].add2(m, r);
+            } else {
+                acc[2 * i + 0].template add2<VAR == kVarNoSub>(pick<0>(r, m), pick<1>(r, m));
+                acc[2 * i + 1].template add2<VAR == kVarNoSub>(pick<2>(r, m), pick<3>(r, m));
+            }
+        }
     }
 }
 

@@ -113,7 +113,8 @@ __device__ __forceinline__ void excise_cell_stream(const CUtensorMap* tmap, cons
 // 128 registers with the sums spilled to local memory 409.
 constexpr int stream_max_regs(int nlev) { return nlev == 1 ? 128 : nlev == 2 ? 200 : 232; }
 
-template <int L, int NLEV, bool CHUNKED>
+// VAR: kVarProduct in the product library; the bench library instantiates kVarMemOnly (sk_device.cuh).
+template <int L, int NLEV, bool CHUNKED, int VAR = kVarProduct>
 __global__ void __maxnreg__(stream_max_regs(NLEV))
 sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) {
     constexpr int RPW = 32 / L;                    // rows covered by one warp-wide 128-bit read
@@ -179,7 +180,7 @@ sk_stream_kernel(const __grid_constant__ CUtensorMap tmap, const FrameParams p) 
         const uint32_t src = ring + s * kTileBytes + lane_off;
         mbar_wait(bars + 8 * s, parity);
 #pragma unroll
-        for (int i = 0; i < NLD; ++i) accumulate16(acc, lds128(src + i * RPW * W), kc);
+        for (int i = 0; i < NLD; ++i) accumulate16<AccChain2, VAR>(acc, lds128(src + i * RPW * W), kc);
         __syncwarp();                              // every lane has consumed this slot: refill it
         if (lane == 0 && g + kStages < total) {
             mbar_expect_tx(bars + 8 * s, kTileBytes);

@@ -32,6 +32,30 @@ def test_header_symbols_are_exported(sk):
         assert getattr(raw, n) is not None
 
 
+def test_product_has_no_measurement_or_override_entries(sk):
+    """The product boundary carries no measurement kernels and no process-wide knobs ("no
+    globals"): those live in libsk_b200_bench.so, which loads and exports what csrc/bench/sk_bench.h declares."""
+    names = declared_symbols()
+    assert not [n for n in names if n.startswith("sk_debug")]
+    raw = C.CDLL(sk.LIB_PATH)
+    for gone in ("sk_debug_set_plan", "sk_debug_get_plan", "sk_debug_loop_ceiling", "sk_debug_pipe_rate"):
+        assert not hasattr(raw, gone)
+    from paper_1808_10365_b200 import benchlib
+    text = open(os.path.join(ROOT, "paper_1808_10365_b200", "csrc", "bench", "sk_bench.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(skb_[a-z_0-9]+)\s*\(", text)))
+    assert set(declared) == set(benchlib.SYMBOLS)
+    braw = C.CDLL(benchlib.LIB_PATH)
+    for n in declared:
+        assert getattr(braw, n) is not None
+    one = C.c_void_p(256)
+    L = benchlib.lib()
+    assert L.skb_loop_ceiling(0, 12, 0, one, one, None, None) == -2          # argument errors need no device
+    assert L.skb_loop_ceiling(1, 12, 10, one, one, None, None) == -5         # the memory-only variant has no loop form
+    assert L.skb_stream_workspace_bytes(49152, 1, 2048, 256) == 192 * 8 * 8 + 192 * 4
+    assert L.skb_stream_workspace_bytes(49152, 1, 2048, 512) == 0
+
+
 def test_version_and_strerror(sk):
     assert sk.sk_version() >= 100
     assert sk.sk_strerror(0) == "ok"

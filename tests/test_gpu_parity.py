@@ -79,9 +79,9 @@ SHAPES = [
 @pytest.fixture(autouse=True)
 def automatic_plan(sk):
     """Every test starts from, and leaves behind, the library's automatic kernel choice."""
-    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+    sk.plan_override(sk.SK_PLAN_AUTO, 0)
     yield
-    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+    sk.plan_override(sk.SK_PLAN_AUTO, 0)
 
 
 PATHS = {"tma": 0, "ldg": 1}          # SK_PLAN_AUTO (the TMA stream kernel where it applies), SK_PLAN_LDG
@@ -90,8 +90,9 @@ PATHS = {"tma": 0, "ldg": 1}          # SK_PLAN_AUTO (the TMA stream kernel wher
 @pytest.fixture(params=["tma", "ldg"])
 def vector_path(request, sk):
     """Both vector kernels (TMA-staged and direct 128-bit loads) must satisfy every parity test:
-    sk_debug_set_plan (the header's test-only entry) forces the direct-load kernel."""
-    sk.sk_debug_set_plan(PATHS[request.param], 0)
+    plan_override makes every fused call pass SK_FRAME_PLAN_LDG (include/sk_b200.h), which forces the
+    direct-load kernel for that call."""
+    sk.plan_override(PATHS[request.param], 0)
     return request.param
 
 
@@ -332,7 +333,7 @@ def test_vector_paths_bit_identical(sk):
         data = sk_synth.random_bytes(T, F, E, seed=21).cuda()
         res = {}
         for path in ("tma", "ldg"):
-            sk.sk_debug_set_plan(PATHS[path], 0)
+            sk.plan_override(PATHS[path], 0)
             res[path] = sk.sk_frame(data, M, n_sigma=2.0, sk_mean=0.4, want_sums=True)
         torch.cuda.synchronize()
         a, b = res["tma"], res["ldg"]
@@ -344,7 +345,7 @@ def test_vector_paths_bit_identical(sk):
 
 def test_sk_independent_of_slab_width_and_kernel(sk):
     """The sum over inputs follows a canonical tree over the input indices: every slab width
-    (sk_debug_set_plan's lanes), both vector kernels, the unfused path and the scalar kernel (misaligned
+    (SK_FRAME_PLAN_LANES), both vector kernels, the unfused path and the scalar kernel (misaligned
     pointer) give the same SK bit for bit, receiver subsets and ragged E included."""
     for (T, F, E, M) in [(512, 2, 2048, 128), (384, 3, 528, 96), (256, 1, 4096 + 48, 64)]:
         data = sk_synth.random_bytes(T, F, E, seed=31)
@@ -360,10 +361,10 @@ def test_sk_independent_of_slab_width_and_kernel(sk):
             S1, S2 = sk.sk_power_sums(d, M)
             for lanes in (16, 8, 4, 2, 1):
                 for path in ("tma", "ldg"):
-                    sk.sk_debug_set_plan(PATHS[path], lanes)
+                    sk.plan_override(PATHS[path], lanes)
                     got = sk.sk_frame(d, M, **kw).SK
                     assert torch.equal(got.view(torch.int32), ref.view(torch.int32)), (T, F, E, M, kw.keys(), lanes, path)
-            sk.sk_debug_set_plan(0, 0)
+            sk.plan_override(0, 0)
             un = sk.sk_combine(S1, S2, M, **kw)
             assert torch.equal(un.view(torch.int32), ref.view(torch.int32)), "combine"
 
@@ -564,9 +565,9 @@ def test_plan_keeps_tma_coordinates_non_negative(sk):
     """The coordinates of a TMA box are signed 32-bit: a frame whose rows are 2^31 bytes or longer
     (F*E, still a legal shape) must not be given to the stream kernel, whose upper boxes would come
     back zero-filled; one just below that still is.  (Plan only: such a frame is >= 64 GiB.)"""
-    assert sk.sk_debug_get_plan(32, 2047, 1 << 20, 32)[2] == 32        # F*E + 256 <= 2^31: TMA stream kernel
-    assert sk.sk_debug_get_plan(32, 2048, 1 << 20, 32)[2] == 0         # F*E = 2^31: direct-load kernel
-    assert sk.sk_debug_get_plan(32, 4095, 1 << 20, 32)[2] == 0
+    assert sk.sk_frame_plan(32, 2047, 1 << 20, 32)[2] == 32        # F*E + 256 <= 2^31: TMA stream kernel
+    assert sk.sk_frame_plan(32, 2048, 1 << 20, 32)[2] == 0         # F*E = 2^31: direct-load kernel
+    assert sk.sk_frame_plan(32, 4095, 1 << 20, 32)[2] == 0
 
 
 def test_host_entry_point(sk, oracle):
@@ -649,12 +650,12 @@ def test_tensor_map_refusal_falls_back_to_direct_loads(sk, oracle):
     ragged = sk_synth.random_bytes(3000, 1, 512, seed=77).cuda()      # M = 1000: the ragged stream kernel
     want_r = sk.sk_frame(ragged, 1000, sk_mean=0.4)
     n0 = sk.sk_launch_count()
-    sk.sk_debug_set_plan(sk.SK_PLAN_NO_TMAP, 0)
-    assert sk.sk_debug_get_plan(T, F, E, M, nlev=nlev)[2] != 0        # the plan still asks for the stream kernel
+    sk.plan_override(sk.SK_PLAN_NO_TMAP, 0)
+    assert sk.sk_frame_plan(T, F, E, M, nlev=nlev)[2] != 0        # the plan still asks for the stream kernel
     got1 = sk.sk_frame(d1.clone(), 256, n_sigma=4.0, sk_mean=0.913, want_sums=True, zero_flagged=True)
     got = sk.sk_frame_multi(d1, M, nlev, n_sigma=4.0, sk_means=means, zero_flagged=True)
     got_r = sk.sk_frame(ragged, 1000, sk_mean=0.4)
-    sk.sk_debug_set_plan(sk.SK_PLAN_AUTO, 0)
+    sk.plan_override(sk.SK_PLAN_AUTO, 0)
     torch.cuda.synchronize()
     assert sk.sk_launch_count() - n0 == 1 + (nlev + nlev) + 1       # fused; one pass and one excision per length; fused
     assert torch.equal(got1.SK.view(torch.int32), want1.SK.view(torch.int32)) and torch.equal(got1.mask, want1.mask)
@@ -700,15 +701,35 @@ def test_eq13_mode(sk, oracle, T, F, E, M):
         np.testing.assert_allclose(got, c * sk14, rtol=2e-6, atol=2e-7)
 
 
-def test_measurement_entries(sk):
-    """sk_debug_loop_ceiling / sk_debug_pipe_rate (measurement only): they run and return plausible
-    cycle counts (one instruction per 1..4 cycles; the loop's 3.98 instructions per 32 samples cannot
-    take fewer than 3.98 cycles)."""
-    c = sk.sk_debug_loop_ceiling(12, 20)
+def test_bench_library_entries(sk, oracle):
+    """libsk_b200_bench.so (measurement only, csrc/bench/sk_bench.h; not part of the product library): the
+    loop ceiling and pipe rates return plausible cycle counts (one instruction per 1..4 cycles; the loop's
+    3.98 instructions per 32 samples cannot take fewer than 3.98 cycles), every removal variant is cheaper
+    than the full loop, and skb_stream with the product's loop body IS the product kernel: same SK and mask,
+    bit for bit, as sk_frame (so the memory-only variant differs from the product by its arithmetic alone)."""
+    from paper_1808_10365_b200 import benchlib
+    c = benchlib.loop_ceiling(12, 20)
     assert 3.98 < c < 12.0
-    for mode, name in enumerate(sk.PIPE_MODES):
-        r = sk.sk_debug_pipe_rate(mode, 16)
+    for name in ("no_fadd2", "no_prmt", "no_unpack"):
+        v = benchlib.loop_ceiling(12, 20, variant=benchlib.VARIANTS[name])
+        assert 2.0 < v < c, (name, v, c)
+    for mode, name in enumerate(benchlib.PIPE_MODES):
+        r = benchlib.pipe_rate(mode, 16)
         assert 0.9 < r < 8.0, (name, r)
+    T, F, E, M = 2048, 2, 2048, 256
+    d = sk_synth.random_bytes(T, F, E, seed=5).cuda()
+    want = sk.sk_frame(d, M, n_sigma=5.0, sk_mean=1.0)
+    SK = torch.empty_like(want.SK)
+    mask = torch.empty_like(want.mask)
+    ws = benchlib.stream_workspace(T, F, E, M, d.device)
+    for ready in (False, True):
+        benchlib.stream(benchlib.VAR_PRODUCT, d, M, SK, mask, ws, inputs_ready=ready)
+        torch.cuda.synchronize()
+        assert torch.equal(SK.view(torch.int32), want.SK.view(torch.int32)) and torch.equal(mask, want.mask)
+        assert int(ws.abs().sum().item()) == 0
+    benchlib.stream(benchlib.VAR_MEMONLY, d, M, SK, mask, ws)      # runs; its outputs mean nothing
+    torch.cuda.synchronize()
+    assert int(ws.abs().sum().item()) == 0
 
 
 @pytest.mark.parametrize("first_n", [16, 64, 300, 2048])
@@ -732,7 +753,7 @@ def test_ragged_blocks_pipelined_with_excision(sk, oracle):
     """Long blocks that are not a whole number of tiles (the ragged stream kernel), back to back with
     SK_FRAME_INPUTS_READY and in-place excision: every frame's SK, mask and bytes are the oracle's."""
     T, F, E, M = 3000, 2, 2048, 300
-    assert sk.sk_debug_get_plan(T, F, E, M, inputs_ready=True)[2] != 0          # a TMA kernel, not the direct-load one
+    assert sk.sk_frame_plan(T, F, E, M, inputs_ready=True)[2] != 0          # a TMA kernel, not the direct-load one
     frames = [sk_synth.random_bytes(T, F, E, seed=300 + i) for i in range(4)]
     for fr in frames:
         fr[M:2 * M, 0, :] = 0x88
@@ -774,7 +795,7 @@ def test_randomised_shapes_and_flags(sk, oracle):
         zero, sums, ready = bool(rng.random() < 0.5), bool(rng.random() < 0.5), bool(rng.random() < 0.5)
         path, lanes = int(rng.choice([0, 0, 0, 1])), int(rng.choice([0, 0, 0, 16, 8, 4, 2, 1]))
         sk_mean, ns = float(rng.choice([0.4, 0.9, 1.0])), float(rng.choice([1.0, 3.0]))
-        sk.sk_debug_set_plan(path, lanes)
+        sk.plan_override(path, lanes)
         ref = oracle.frame(data.numpy(), M, n_sigma=ns, sk_mean=sk_mean, zero_flagged=zero, **kw)
         d = data.cuda()
         torch.cuda.synchronize()

@@ -82,7 +82,7 @@ def _cases():
 def test_noalloc_equals_sk_frame_back_to_back(sk):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
-    sk.sk_debug_set_plan(0, 0)
+    sk.plan_override(0, 0)
     dev = torch.device("cuda", torch.cuda.current_device())
     cases = _cases()
     # the existing path first, each frame on its own copy and with its own workspace
@@ -117,7 +117,7 @@ def test_noalloc_same_frame_twice_in_a_row(sk):
     """The plainest form of the requirement: one frame, two calls in a row, both equal to sk_frame."""
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
-    sk.sk_debug_set_plan(0, 0)
+    sk.plan_override(0, 0)
     dev = torch.device("cuda", torch.cuda.current_device())
     host = sk_synth.random_bytes(4096, 4, 1024, seed=44)
     d = host.to(dev)
