@@ -91,22 +91,36 @@ def stored_traffic(name):
     return int(row["dram_bytes_per_launch"]) if row else None
 
 
-def issue_roofline(name, samples_per_launch, achieved_samples_per_s):
-    """Roofline object of a kernel bound by instruction issue rather than HBM (the simulators):
-    the ceiling is one warp instruction per cycle and sub-partition (592 x 1.965 GHz) at the
-    instruction count ncu MEASURED for one launch (smsp__inst_executed.sum, committed under
-    profiles/); ncu's own issue utilisation of that launch is given beside it."""
+# Philox4x32-10 as the oracle fixes it (one 32-bit word per component, ten rounds): 20 IMAD.WIDE per call
+# of 4 words = 2 complex samples, each holding the half-rate fmaheavy pipe of a sub-partition for 4 cycles
+# (bench.py --op ceiling: IDP / FFMA2 / IMAD class instructions issue every 2 cycles per warp, a wide multiply
+# is two of them): 40 pipe cycles per complex sample and lane, before any digitising or Box-Muller.
+PHILOX_PIPE_CYCLES_PER_SAMPLE = 40.0
+
+
+def method_roofline(name, samples_per_launch, achieved_samples_per_s, bytes_written_per_sample):
+    """Roofline object of the two simulators against what the METHOD needs, not against the kernel's own
+    instruction count: the lower of the HBM rate for the bytes a sample writes and the generator's floor on
+    the fmaheavy pipe (PHILOX_PIPE_CYCLES_PER_SAMPLE).  The kernel's issue utilisation from
+    the committed ncu capture is reported beside it as what it is: IPC, not a fraction of a roofline."""
+    hbm, hbm_src = peaks()
+    philox = 592 * 1.965e9 * 32.0 / PHILOX_PIPE_CYCLES_PER_SAMPLE / 1e9            # Gsamples/s
+    hbm_bound = hbm / bytes_written_per_sample if bytes_written_per_sample else float("inf")
+    peak = min(philox, hbm_bound)
     row = stored_profile(name)
-    if not row:
-        return None
-    inst = float(row["warp_instructions_per_launch"])
-    per32 = inst * 32.0 / samples_per_launch
-    peak = 592 * 1.965e9 * 32.0 / per32 / 1e9
-    return {"bound": "alu", "achieved": achieved_samples_per_s / 1e9, "unit": "Gsamples/s", "peak": peak,
-            "frac": achieved_samples_per_s / 1e9 / peak, "traffic": int(row["dram_bytes_per_launch"]),
-            "warp_instructions_per_32_samples": per32, "ncu_issue_active_pct": float(row["issue_active_pct"]),
-            "peak_source": "issue slots: 592 sub-partitions x 1.965 GHz / (ncu smsp__inst_executed.sum per sample), "
-                           "profiles/" + row["source"]}
+    out = {"bound": "alu" if philox <= hbm_bound else "hbm", "achieved": achieved_samples_per_s / 1e9, "unit": "Gsamples/s",
+           "peak": peak, "frac": achieved_samples_per_s / 1e9 / peak,
+           "traffic": int(row["dram_bytes_per_launch"]) if row else None,
+           "peak_source": "min(Philox4x32-10 floor: 592 sub-partitions x 1.965 GHz x 32 lanes / %g fmaheavy cycles per "
+                          "sample = %.0f Gsamples/s; HBM write at %g B per sample: %s)"
+                          % (PHILOX_PIPE_CYCLES_PER_SAMPLE, philox, bytes_written_per_sample,
+                             "%.0f Gsamples/s" % hbm_bound if bytes_written_per_sample else "none, nothing is stored"),
+           "frac_of_hbm_write_roofline": (achieved_samples_per_s / 1e9 / hbm_bound) if bytes_written_per_sample else None}
+    if row:
+        per32 = float(row["warp_instructions_per_launch"]) * 32.0 / samples_per_launch
+        out["issue"] = {"warp_instructions_per_32_samples": per32, "ncu_issue_active_pct": float(row["issue_active_pct"]),
+                        "note": "IPC of the kernel's own instruction stream (profiles/%s), not a roofline" % row["source"]}
+    return out
 
 
 def sm_ceiling(sk, torch, dev, sm_mhz, sm_max_mhz, achieved_samples_per_s, warps=12):
@@ -470,7 +484,7 @@ def run_sim(args):
         "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
         "dtype": "u32->u8", "config": {"workload": cfg.name + " shape, per-input sigma ~ U[1.5,3.5]",
                                        "null_mean": float(mean[0].item()), "null_var": float(var[0].item())},
-        "roofline": issue_roofline("sim", cfg.nbytes, cfg.nbytes / (ms * 1e-3)),
+        "roofline": method_roofline("sim", cfg.nbytes, cfg.nbytes / (ms * 1e-3), 1.0),
         "gpu_launches": int(sk.sk_launch_count() - n0) }))
 
 
@@ -499,7 +513,7 @@ def run_cm(args):
         "dtype": "f64", "config": {"workload": f"App. A: {D} datasets x n={M} x N={N}, common-mode amplitude {amp}",
                                    "mean": float(mean[0].item()), "var": float(var[0].item()),
                                    "n_eff": 4.0 / (M * float(var[0].item()))},
-        "roofline": issue_roofline("cm", D * M * N, D * M * N / (ms * 1e-3)),
+        "roofline": method_roofline("cm", D * M * N, D * M * N / (ms * 1e-3), 0.0),
         "gpu_launches": int(sk.sk_launch_count() - n0)}))
 
 
@@ -567,7 +581,8 @@ def run_fig6(args):
 
 def run_aux(args):
     """--op rebin|single: one of the small HBM-bound kernels beside the hot path, on S1/S2 arrays of
-    config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), two rotating copies."""
+    config 4's size (16384 cells x 2048 inputs: 256 MiB for the pair, > L2), five rotating copies (1.25 GiB,
+    ten times the L2, so that no launch finds a part of its input still resident)."""
     import torch
     import paper_1808_10365_b200 as sk
     import sk_synth
@@ -577,20 +592,21 @@ def run_aux(args):
     S1, S2 = sk.sk_power_sums(frame, cfg.M)
     del frame
     reps = 8                                               # config 2's 2048 cells x 8 = config 4's 16384
-    sums = [(S1.repeat(reps, 1, 1), S2.repeat(reps, 1, 1)) for _ in range(2)]
+    ncopies = 5
+    sums = [(S1.repeat(reps, 1, 1), S2.repeat(reps, 1, 1)) for _ in range(ncopies)]
     B, F, E = sums[0][0].shape
     n = B * F * E
     fn = (lambda a, b: sk.sk_rebin_sums(a, b, cfg.M, 2)) if args.op == "rebin" else (lambda a, b: sk.sk_single(a, b, cfg.M))
     alg = n * 8 + (n * 8 // 2 if args.op == "rebin" else n * 4)
     K, W = max(args.steps, 50), max(args.warmup, 3)
     for i in range(W):
-        fn(*sums[i % 2])
+        fn(*sums[i % ncopies])
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = sk.sk_launch_count()
     e0.record()
     for i in range(K):
-        fn(*sums[i % 2])
+        fn(*sums[i % ncopies])
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / K
@@ -600,7 +616,7 @@ def run_aux(args):
         "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "data": "synthetic",
         "dtype": "u32" if args.op == "rebin" else "u32->f64->f32",
         "config": {"workload": f"S1,S2 [{B}][{F}][{E}] uint32 (config 4's size), M={cfg.M}",
-                   "l2": "two rotating copies, 256 MiB each"},
+                   "l2": "%d rotating copies, 256 MiB each" % ncopies},
         "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": alg / (ms * 1e-3) / 1e9 / peak, "traffic": stored_traffic(args.op), "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg},
