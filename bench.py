@@ -1072,6 +1072,30 @@ def main():
                                 "sample": f"{n} passes over {blocks} of {cfg.B} blocks of {cfg.name} "
                                           f"({host.size} samples each), {dt:.1f} s, single thread; "
                                           f"host has {os.cpu_count()} cores"}
+        # SURVEY 8(d)'s optional second baseline: the same oracle, unchanged, on every host core at once (one
+        # thread per core, each on its own slab of whole blocks; ctypes releases the GIL around the C call)
+        cores = os.cpu_count() or 1
+        if cores > 1 and blocks >= cores:
+            from concurrent.futures import ThreadPoolExecutor
+            per = blocks // cores
+            slabs = [host[i * per * cfg.M:(i + 1) * per * cfg.M] for i in range(cores)]
+            secs = max(1.0, args.cpu_seconds / 2)
+            t0 = time.perf_counter()
+
+            def passes(h):
+                k = 0
+                while True:
+                    sk_oracle.frame(h, cfg.M, n_sigma=n_sigma, sk_mean=sk_mean)
+                    k += 1
+                    if time.perf_counter() - t0 >= secs:
+                        return k * h.size
+
+            with ThreadPoolExecutor(cores) as ex:
+                done = sum(ex.map(passes, slabs))
+            dt = time.perf_counter() - t0
+            line["cpu_baseline"]["all_cores"] = {"value": done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                                 "sample": f"{cores} threads, each repeating its own {per}-block slab of the "
+                                                           f"same frame for {dt:.1f} s"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
