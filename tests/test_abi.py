@@ -56,6 +56,24 @@ def test_product_has_no_measurement_or_override_entries(sk):
     assert L.skb_stream_workspace_bytes(49152, 1, 2048, 512) == 0
 
 
+def test_plan_override_is_per_call(sk):
+    """The SK_FRAME_PLAN_* bits act on the call that carries them and leave nothing behind in the library
+    (sk_frame_plan is a pure query, so this needs no device)."""
+    auto = sk.sk_frame_plan(49152, 1, 2048, 256, flags=0)
+    for lanes in (1, 2, 4, 8, 16):
+        assert sk.sk_frame_plan(49152, 1, 2048, 256, flags=sk.plan_flags(lanes=lanes))[0] == lanes
+        assert sk.sk_frame_plan(49152, 1, 2048, 256, flags=0) == auto
+    assert sk.sk_frame_plan(49152, 1, 2048, 256, flags=sk.plan_flags(sk.SK_PLAN_LDG))[2] == 0     # direct-load kernel
+    assert sk.sk_frame_plan(49152, 1, 2048, 256, flags=3 << 12) == auto                            # 3 lanes: not a width, ignored
+    assert sk.plan_flags(sk.SK_PLAN_LDG, 8) == (1 << 8) | (8 << 12) and sk.plan_flags(sk.SK_PLAN_NO_TMAP) == 1 << 9
+    sk.plan_override(sk.SK_PLAN_LDG, 4)                      # the Python-side default for calls made through the binding
+    try:
+        assert sk.sk_frame_plan(49152, 1, 2048, 256)[0] == 4
+    finally:
+        sk.plan_override(0, 0)
+    assert sk.sk_frame_plan(49152, 1, 2048, 256) == auto
+
+
 def test_version_and_strerror(sk):
     assert sk.sk_version() >= 100
     assert sk.sk_strerror(0) == "ok"
