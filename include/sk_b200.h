@@ -178,6 +178,20 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
                   uint8_t* d_data, float* d_SK, uint8_t* d_mask,
                   void* workspace, size_t workspace_bytes, void* stream);
 
+/* sk_frame_host for a QUEUE of frames: h_frames is a HOST array of nframes host pointers (T*F*E bytes each,
+ * pinned memory recommended); h_SK float32 [nframes][T/M][F] and h_mask uint8 [nframes][T/M][F] receive the
+ * results of frame i at index i.  Upload, kernel and read-back of all frames are enqueued back to back on
+ * `stream` and the call waits ONCE at the end, so the host-to-device link is never idle while the host turns
+ * a call around (sk_frame_host waits after every frame).  One staging frame d_data and one set of device
+ * outputs d_SK / d_mask / workspace serve all frames (stream order keeps them safe).  With
+ * SK_FRAME_ZERO_FLAGGED every h_frames[i] is overwritten with its excised frame.  Results per frame are those
+ * of sk_frame_host.  Errors as for sk_frame_host; after a launch or copy error the frames not yet enqueued are
+ * dropped and the call still waits for what it had enqueued. */
+int sk_frames_host(uint8_t* const* h_frames, uint32_t nframes, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                   const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean, int flags,
+                   float* h_SK, uint8_t* h_mask, uint8_t* d_data, float* d_SK, uint8_t* d_mask,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- outputs next to the hot path ---------------------------------- */
 
 /* Several integration lengths from one pass ("a variety of integration

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libsk_b200.so")
 
 SYMBOLS = ("sk_power_sums", "sk_combine", "sk_flag", "sk_frame_workspace_bytes", "sk_frame",
            "sk_frame_noalloc",
-           "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_rebin_sums", "sk_single",
+           "sk_frame_multi_workspace_bytes", "sk_frame_multi", "sk_frame_host", "sk_frames_host", "sk_rebin_sums", "sk_single",
            "sk_significance", "sk_sim_digitised", "sk_sim_common_mode", "sk_moments", "sk_strerror", "sk_version",
            "sk_launch_count", "sk_frame_plan")
 
@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
     L.sk_frame_noalloc.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp]
     L.sk_frame_noalloc.restype = i32
     L.sk_frame_host.argtypes = [vp, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_frames_host.argtypes = [vp, u32, u32, u32, u32, u32, vp, u32, f32, f32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sk_frames_host.restype = i32
     L.sk_frame_multi_workspace_bytes.argtypes = [u32, u32, u32, u32, u32]
     L.sk_frame_multi_workspace_bytes.restype = sz
     L.sk_frame_multi.argtypes = [vp, u32, u32, u32, u32, u32, vp, u32, f32, vp, i32, vp, vp, vp, sz, vp]
@@ -453,4 +455,35 @@ def sk_frame_host(h_data: torch.Tensor, M: int, h_SK: torch.Tensor, h_mask: torc
                                    sk_mean, int(bool(zero_flagged)) | _plan_flags, h_SK.data_ptr(), h_mask.data_ptr(),
                                    d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
                                    workspace.numel() * workspace.element_size(), ts.cuda_stream), "sk_frame_host")
+    return h_SK, h_mask
+
+
+def sk_frames_host(h_frames, M: int, h_SK: torch.Tensor, h_mask: torch.Tensor, d_data: torch.Tensor,
+                   d_SK: torch.Tensor, d_mask: torch.Tensor, subset=None, first_n=None, n_sigma: float = 3.0,
+                   sk_mean: float = 1.0, zero_flagged: bool = False, workspace: Optional[torch.Tensor] = None, stream=None):
+    """sk_frame_host for a queue of frames (include/sk_b200.h): h_frames is a list of host tensors uint8
+    [T][F][E] (pinned recommended), h_SK float32 / h_mask uint8 [len(h_frames)][T/M][F] receive the results;
+    uploads, kernels and read-backs are enqueued back to back and the call waits once at the end."""
+    n = len(h_frames)
+    if n == 0 or any(t.is_cuda or t.dtype != torch.uint8 or not t.is_contiguous() or t.shape != h_frames[0].shape
+                     for t in h_frames) or h_SK.is_cuda or h_mask.is_cuda:
+        raise SKError("h_frames must be equal-shaped contiguous uint8 host tensors, h_SK / h_mask host tensors")
+    T, F, E = h_frames[0].shape
+    B = T // M if M else 0
+    if (tuple(h_SK.shape) != (n, B, F) or tuple(h_mask.shape) != (n, B, F) or h_SK.dtype != torch.float32
+            or h_mask.dtype != torch.uint8 or not h_SK.is_contiguous() or not h_mask.is_contiguous()):
+        raise SKError("h_SK float32 / h_mask uint8 must be contiguous [nframes][T/M][F]")
+    _dev(d_data, torch.uint8, "d_data")
+    ts = _torch_stream(stream, d_data.device)
+    with torch.cuda.stream(ts):
+        sub = _subset(subset, E, d_data.device)
+        if sub is None and first_n is None:
+            first_n = E
+        if workspace is None:
+            workspace = workspace_for(T, F, E, M, d_data.device, ts.cuda_stream)
+        ptrs = (C.c_void_p * n)(*[t.data_ptr() for t in h_frames])
+        _check(lib().sk_frames_host(C.cast(ptrs, C.c_void_p), n, T, F, E, M, _ptr(sub), int(first_n or 0), n_sigma, sk_mean,
+                                    int(bool(zero_flagged)) | _plan_flags, h_SK.data_ptr(), h_mask.data_ptr(),
+                                    d_data.data_ptr(), d_SK.data_ptr(), d_mask.data_ptr(), workspace.data_ptr(),
+                                    workspace.numel() * workspace.element_size(), ts.cuda_stream), "sk_frames_host")
     return h_SK, h_mask

@@ -642,6 +642,43 @@ int sk_frame_host(uint8_t* h_data, uint32_t T, uint32_t F, uint32_t E, uint32_t 
     return rc;
 }
 
+int sk_frames_host(uint8_t* const* h_frames, uint32_t nframes, uint32_t T, uint32_t F, uint32_t E, uint32_t M,
+                   const uint8_t* subset, uint32_t first_n, float n_sigma, float sk_mean, int flags, float* h_SK,
+                   uint8_t* h_mask, uint8_t* d_data, float* d_SK, uint8_t* d_mask, void* workspace,
+                   size_t workspace_bytes_given, void* stream) {
+    if (!h_frames || !h_SK || !h_mask || !d_data || !d_SK || !d_mask) return SK_ERR_NULL;
+    if (nframes == 0) return SK_ERR_SHAPE;
+    for (uint32_t i = 0; i < nframes; ++i)
+        if (!h_frames[i]) return SK_ERR_NULL;
+    // every argument error is reported before the first upload is enqueued
+    if (int rc = check_shape(T, F, E, M)) return rc;
+    if (int rc = check_frame_args(subset, E, first_n, n_sigma, &sk_mean, 1, true)) return rc;
+    if (vector_ok(d_data, E) && (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7u) ||
+                                 workspace_bytes_given < workspace_bytes(T / M, F, E, 1)))
+        return SK_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)T * F * E, cells = (size_t)(T / M) * F;
+    const int keep = flags & ~SK_FRAME_INPUTS_READY;
+    int rc = SK_OK;
+    // upload i, kernel i, read-back i, upload i+1, ...: stream order keeps the one staging frame and the one
+    // set of device outputs safe, and the host is not in the loop, so the link never waits for it
+    for (uint32_t i = 0; i < nframes && rc == SK_OK; ++i) {
+        cudaError_t e = cudaMemcpyAsync(d_data, h_frames[i], bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { rc = (int)e; break; }
+        rc = sk_frame(d_data, T, F, E, M, subset, first_n, n_sigma, sk_mean, keep, d_SK, d_mask, nullptr, nullptr,
+                      workspace, workspace_bytes_given, stream);
+        if (rc != SK_OK) break;
+        e = cudaMemcpyAsync(h_SK + (size_t)i * cells, d_SK, cells * sizeof(float), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_mask + (size_t)i * cells, d_mask, cells, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && (flags & SK_FRAME_ZERO_FLAGGED))
+            e = cudaMemcpyAsync(h_frames[i], d_data, bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) rc = (int)e;
+    }
+    const cudaError_t e = cudaStreamSynchronize(st);       // wait for whatever was enqueued, also after an error
+    if (rc == SK_OK && e != cudaSuccess) rc = (int)e;
+    return rc;
+}
+
 int sk_rebin_sums(const uint32_t* S1, const uint32_t* S2, uint32_t B, uint32_t F, uint32_t E, uint32_t M,
                   uint32_t factor, uint32_t* S1out, uint32_t* S2out, void* stream) {
     if (!S1 || !S2 || !S1out || !S2out) return SK_ERR_NULL;

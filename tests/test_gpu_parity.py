@@ -561,6 +561,37 @@ def test_argument_errors(sk):
         sk.sk_frame(torch.zeros(64, 1, 32, dtype=torch.uint8), 32)          # CPU tensor: no fallback
 
 
+def test_host_queue_entry_point(sk, oracle):
+    """sk_frames_host: a queue of host frames through one staging buffer, one wait at the end; every frame's
+    SK, mask and (with excision) bytes are the oracle's, and equal to sk_frame_host's frame by frame."""
+    T, F, E, M = 1024, 2, 512, 128
+    frames = [sk_synth.random_bytes(T, F, E, seed=500 + i) for i in range(5)]
+    for fr in frames:
+        fr[M:2 * M, 1, :] = 0x88                              # a cell that is certainly flagged around 0.4
+    pinned = [fr.clone().pin_memory() for fr in frames]
+    B = T // M
+    h_SK = torch.empty(len(frames), B, F, dtype=torch.float32).pin_memory()
+    h_mask = torch.empty(len(frames), B, F, dtype=torch.uint8).pin_memory()
+    d_data = torch.empty(T, F, E, dtype=torch.uint8, device="cuda")
+    d_SK = torch.empty(B, F, dtype=torch.float32, device="cuda")
+    d_mask = torch.empty(B, F, dtype=torch.uint8, device="cuda")
+    sk.sk_frames_host(pinned, M, h_SK, h_mask, d_data, d_SK, d_mask, n_sigma=2.0, sk_mean=0.4, zero_flagged=True)
+    one_SK = torch.empty(B, F, dtype=torch.float32).pin_memory()
+    one_mask = torch.empty(B, F, dtype=torch.uint8).pin_memory()
+    for i, fr in enumerate(frames):
+        ref = oracle.frame(fr.numpy(), M, n_sigma=2.0, sk_mean=0.4, zero_flagged=True)
+        assert_sk_close(h_SK[i].numpy(), ref["SK"])
+        np.testing.assert_array_equal(h_mask[i].numpy(), ref["mask"])
+        np.testing.assert_array_equal(pinned[i].numpy(), ref["data"])
+        assert 0 < ref["mask"].sum() < ref["mask"].size
+        again = fr.clone().pin_memory()
+        sk.sk_frame_host(again, M, one_SK, one_mask, d_data, d_SK, d_mask, n_sigma=2.0, sk_mean=0.4, zero_flagged=True)
+        assert torch.equal(one_SK.view(torch.int32), h_SK[i].view(torch.int32)) and torch.equal(one_mask, h_mask[i])
+        assert torch.equal(again, pinned[i])
+    with pytest.raises(sk.SKError):
+        sk.sk_frames_host([], M, h_SK, h_mask, d_data, d_SK, d_mask)
+
+
 def test_plan_keeps_tma_coordinates_non_negative(sk):
     """The coordinates of a TMA box are signed 32-bit: a frame whose rows are 2^31 bytes or longer
     (F*E, still a legal shape) must not be given to the stream kernel, whose upper boxes would come
